@@ -1,0 +1,133 @@
+/* cm_dg.h -- C ABI of the B200-native nodal-DG right-hand side for atmospheric LES
+ * (hot path of arXiv 2110.00853, "Large-eddy simulations with ClimateMachine").
+ *
+ * P:L<n> below = line n of the paper text.  The library evaluates, in fp64 on one GPU,
+ *
+ *     dY/dt = -div(F1(Y) + F2(Y, grad Y)) + S(Y)                                  eq. (16)
+ *
+ * for Y = [rho, rho*u, rho*v, rho*w, rho*e_tot, (rho*q_tot)] on a structured brick of hexahedral
+ * elements with (N+1)^3 Legendre-Gauss-Lobatto nodes each (eq. 17), discretised by the nodal
+ * discontinuous-Galerkin method of eq. (26)/(32) with the Rusanov flux (eq. 27), the
+ * BR1 auxiliary gradient (eq. 28-31), the Smagorinsky-Lilly closure (eq. 33-38),
+ * reflecting free-slip walls (App. A3) and the 2N-storage LSRK54 scheme.
+ *
+ * Conventions
+ *   - Every pointer is tagged HOST or DEVICE.  Nothing here is a torch type; the caller allocates device
+ *     memory however it likes (the Python binding uses torch.empty(..., device="cuda")).
+ *   - State layout (DEVICE and the *_host variants alike): structure of arrays, fp64,
+ *         Q[v * field_stride + e * np + n],   v = rho, rho*u, rho*v, rho*w, rho*e_tot, [rho*q_tot]
+ *     e = element in LIBRARY order (0 <= e < n_elem), n = i + Nq*(j + Nq*k) with i along x (xi) fastest,
+ *     Nq = N+1, np = Nq^3.  cm_dg_layout() reports field_stride (>= n_elem*np, a multiple of 32 doubles)
+ *     and lex_of_elem[e] = ex + Ex*(ey + Ey*ez), the lexicographic id of library element e (the library
+ *     orders elements in small spatial tiles so that face neighbours stay close in memory / in L2).
+ *   - All calls on one ctx are issued on the CUDA stream given to cm_dg_setup (0 = legacy default stream).
+ *     cm_dg_rhs / cm_dg_lsrk_step / cm_dg_gradient are asynchronous and never synchronise;
+ *     cm_dg_diagnostics, cm_dg_profile_end and the *_host variants synchronise that stream.
+ *   - Return value: CM_DG_OK (0) or a negative code; cm_dg_last_error() gives a thread-local message.
+ *     No exception or abort crosses this boundary.  Non-finite state values are reported by
+ *     cm_dg_diagnostics (n_nonfinite), never trapped.
+ *   - There is NO CPU fallback: without a CUDA device cm_dg_setup fails with CM_DG_ECUDA.
+ */
+#ifndef CM_DG_H
+#define CM_DG_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CM_DG_OK 0
+#define CM_DG_EINVAL (-1) /* bad N / ne / nvar / NULL pointer / non-positive Jacobian / metric identity > 1e-10 */
+#define CM_DG_ENOMEM (-2)
+#define CM_DG_ECUDA (-3)  /* message carries cudaGetErrorString                                            */
+#define CM_DG_ESTATE (-4) /* call not valid for this ctx (e.g. profile_end without profile_begin)          */
+
+typedef struct cm_dg_ctx cm_dg_ctx; /* opaque, library-owned */
+
+/* Problem description (all HOST memory, copied before cm_dg_setup returns). */
+typedef struct {
+  int32_t N;                /* polynomial order, 2..7 (the paper and BASELINE use 4; sweep 3..6)            */
+  int32_t ne[3];            /* Ex, Ey, Ez: structured hexahedral brick                             */
+  double lo[3], hi[3];      /* domain box before warping [m]                                                */
+  int32_t bc[3];            /* per direction: 0 periodic, 1 impenetrable free-slip no-flux wall at both ends */
+  int32_t nvar;             /* 5 dry | 6 with rho*q_tot                                                     */
+  int32_t geom;             /* 0 flat brick | 1 linear-decay terrain warp of z by zsfc_nodes | 2 xyz */
+  const double* zsfc_nodes; /* geom==1: HOST [Ey*Nq][Ex*Nq] surface height at the bottom nodes              */
+  const double* xyz;        /* geom==2: HOST [3][Ne][Np], LEXICOGRAPHIC element order                       */
+  double R_d, c_vd, R_v, c_vv, T_0, I_v0, grav; /* Table 1, eq. (9); Phi = grav * z     */
+  int32_t sgs;              /* 0 inviscid | 1 Smagorinsky-Lilly (eq. 38)                                    */
+  double C_s, Pr_t;         /* Smagorinsky coefficient, turbulent Prandtl number (eq. 36)                   */
+  int32_t use_ref;          /* 1: remove the hydrostatic reference state in the momentum equation (eq. 4)   */
+  const double *ref_rho, *ref_rhoe, *ref_rhoq; /* HOST [Ne][Np] LEXICOGRAPHIC; resting reference state;
+                                                  p_r is derived from them with the library's EOS          */
+  double shf_bottom;        /* W m^-2 prescribed upward energy flux through the z-low wall, 0 = none */
+} cm_dg_params;
+
+/* Conservation integrals and step-size ingredients (eq. 57; eq. 61-62). */
+typedef struct {
+  double mass;          /* sum M rho,        M = w_i w_j w_k |J|                                           */
+  double energy;        /* sum M rho e_tot                                                                  */
+  double water;         /* sum M rho q_tot (0 when nvar == 5)                                               */
+  double kinetic;       /* E_k = (1/2) sum M |u|^2 / sum M                                                  */
+  double max_wavespeed; /* max over nodes of |u| + c                                                        */
+  double min_node_dx;   /* smallest distance between adjacent LGL nodes of the mesh                         */
+  double volume;        /* sum M                                                                            */
+  int64_t n_nonfinite;  /* number of state values that are NaN or +-Inf                                     */
+} cm_dg_diag;
+
+/* Per-kernel device timings gathered between cm_dg_profile_begin and cm_dg_profile_end (CUDA events
+ * recorded on the ctx stream around every launch). */
+typedef struct {
+  int64_t launches_gradient, launches_tendency, launches_other;
+  double ms_gradient, ms_tendency, ms_other;
+} cm_dg_kernel_stats;
+
+/* a0: mesh, LGL nodes/weights, derivative matrix, metric terms (eq. 24), connectivity,
+ * reference state.  `cuda_stream` is a cudaStream_t (NULL = default stream).  On success *out owns all
+ * device scratch (geometry, gradient array, LSRK residual, second state buffer). */
+int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out);
+
+/* Layout of state arrays: n_elem, np, field_stride (doubles) and, if non-NULL, lex_of_elem (HOST, n_elem
+ * int32 entries).  Any output pointer may be NULL. */
+int cm_dg_layout(const cm_dg_ctx* ctx, int64_t* n_elem, int32_t* np, int64_t* field_stride, int32_t* lex_of_elem);
+
+/* Nodal coordinates in library layout: xyz_dev is DEVICE [3][field_stride]. */
+int cm_dg_coords(cm_dg_ctx* ctx, double* xyz_dev);
+
+/* Metric terms as used by the kernels (tests): Ja_dev DEVICE [9][field_stride] with Ja[3*d+c] = J dxi_d/dx_c
+ * (cross-product form), J_dev DEVICE [field_stride] = det(dx/dxi). */
+int cm_dg_metrics(cm_dg_ctx* ctx, double* Ja_dev, double* J_dev);
+
+/* a2: BR1 auxiliary gradient (eq. 28-31): G_dev DEVICE [15][field_stride], G[3*s+c] = d s/d x_c for
+ * s = u, v, w, h_tot, q_tot (q rows are zero when nvar == 5).  Diagnostic entry point: cm_dg_rhs and
+ * cm_dg_lsrk_step run the same kernel but keep its output in a packed internal form. */
+int cm_dg_gradient(cm_dg_ctx* ctx, const double* Q_dev, double* G_dev);
+
+/* a1-a4: dQ := RHS(Q, t) of eq. (32).  Q_dev, dQ_dev DEVICE [nvar][field_stride], distinct buffers. */
+int cm_dg_rhs(cm_dg_ctx* ctx, const double* Q_dev, double* dQ_dev, double t);
+
+/* a1-a5: advance Q by nsteps LSRK54 steps of size dt; every stage is one gradient kernel plus one fused
+ * tendency + low-storage update kernel.  The result is left in Q_dev (if 5*nsteps is odd one device copy
+ * from the internal ping-pong buffer is appended). */
+int cm_dg_lsrk_step(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t nsteps);
+
+/* a6: conservation integrals etc. of Q_dev into *out_host; synchronises the stream. */
+int cm_dg_diagnostics(cm_dg_ctx* ctx, const double* Q_dev, cm_dg_diag* out_host);
+
+/* End-to-end variants on HOST buffers in the same [nvar][field_stride] layout (pinned memory recommended):
+ * host->device copy, the device call above, device->host copy, stream synchronise. */
+int cm_dg_rhs_host(cm_dg_ctx* ctx, const double* Q_host, double* dQ_host, double t);
+int cm_dg_lsrk_step_host(cm_dg_ctx* ctx, double* Q_host, double t, double dt, int32_t nsteps);
+
+/* Kernel timing (measurement support). */
+int cm_dg_profile_begin(cm_dg_ctx* ctx);
+int cm_dg_profile_end(cm_dg_ctx* ctx, cm_dg_kernel_stats* out_host);
+
+void cm_dg_destroy(cm_dg_ctx* ctx);
+const char* cm_dg_last_error(void); /* thread-local, never NULL */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CM_DG_H */

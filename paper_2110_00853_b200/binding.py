@@ -1,0 +1,282 @@
+"""ctypes binding of include/cm_dg.h: argument marshalling only, every step of the path runs in the CUDA
+library.  Function names equal the C entry points; ``CmDg`` is a small convenience wrapper around a ctx."""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "libcm_dg.so")
+
+
+class CmDgError(RuntimeError):
+    pass
+
+
+class _Params(C.Structure):
+    _fields_ = [
+        ("N", C.c_int32), ("ne", C.c_int32 * 3), ("lo", C.c_double * 3), ("hi", C.c_double * 3),
+        ("bc", C.c_int32 * 3), ("nvar", C.c_int32), ("geom", C.c_int32),
+        ("zsfc_nodes", C.c_void_p), ("xyz", C.c_void_p),
+        ("R_d", C.c_double), ("c_vd", C.c_double), ("R_v", C.c_double), ("c_vv", C.c_double),
+        ("T_0", C.c_double), ("I_v0", C.c_double), ("grav", C.c_double),
+        ("sgs", C.c_int32), ("C_s", C.c_double), ("Pr_t", C.c_double), ("use_ref", C.c_int32),
+        ("ref_rho", C.c_void_p), ("ref_rhoe", C.c_void_p), ("ref_rhoq", C.c_void_p),
+        ("shf_bottom", C.c_double),
+    ]
+
+
+class _Diag(C.Structure):
+    _fields_ = [("mass", C.c_double), ("energy", C.c_double), ("water", C.c_double), ("kinetic", C.c_double),
+                ("max_wavespeed", C.c_double), ("min_node_dx", C.c_double), ("volume", C.c_double),
+                ("n_nonfinite", C.c_int64)]
+
+
+class _KStats(C.Structure):
+    _fields_ = [("launches_gradient", C.c_int64), ("launches_tendency", C.c_int64), ("launches_other", C.c_int64),
+                ("ms_gradient", C.c_double), ("ms_tendency", C.c_double), ("ms_other", C.c_double)]
+
+
+EXPORTS = ("cm_dg_setup", "cm_dg_layout", "cm_dg_coords", "cm_dg_metrics", "cm_dg_gradient", "cm_dg_rhs",
+           "cm_dg_lsrk_step", "cm_dg_diagnostics", "cm_dg_rhs_host", "cm_dg_lsrk_step_host",
+           "cm_dg_profile_begin", "cm_dg_profile_end", "cm_dg_destroy", "cm_dg_last_error")
+
+_lib = None
+
+
+def library_path():
+    return _LIBPATH
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIBPATH):
+        raise CmDgError("CUDA library %s is missing: build it with `python -m paper_2110_00853_b200.build` "
+                        "(there is no CPU fallback)" % _LIBPATH)
+    L = C.CDLL(_LIBPATH)
+    vp, dbl, i32, i64 = C.c_void_p, C.c_double, C.c_int32, C.c_int64
+    L.cm_dg_setup.argtypes = [C.POINTER(_Params), vp, C.POINTER(vp)]
+    L.cm_dg_layout.argtypes = [vp, C.POINTER(i64), C.POINTER(i32), C.POINTER(i64), vp]
+    L.cm_dg_coords.argtypes = [vp, vp]
+    L.cm_dg_metrics.argtypes = [vp, vp, vp]
+    L.cm_dg_gradient.argtypes = [vp, vp, vp]
+    L.cm_dg_rhs.argtypes = [vp, vp, vp, dbl]
+    L.cm_dg_lsrk_step.argtypes = [vp, vp, dbl, dbl, i32]
+    L.cm_dg_diagnostics.argtypes = [vp, vp, C.POINTER(_Diag)]
+    L.cm_dg_rhs_host.argtypes = [vp, vp, vp, dbl]
+    L.cm_dg_lsrk_step_host.argtypes = [vp, vp, dbl, dbl, i32]
+    L.cm_dg_profile_begin.argtypes = [vp]
+    L.cm_dg_profile_end.argtypes = [vp, C.POINTER(_KStats)]
+    L.cm_dg_destroy.argtypes = [vp]
+    L.cm_dg_destroy.restype = None
+    L.cm_dg_last_error.restype = C.c_char_p
+    for n in EXPORTS:
+        if n not in ("cm_dg_destroy", "cm_dg_last_error"):
+            getattr(L, n).restype = C.c_int
+    _lib = L
+    return L
+
+
+def cm_dg_last_error():
+    return _load().cm_dg_last_error().decode()
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise CmDgError("%s failed (%d): %s" % (what, rc, cm_dg_last_error()))
+
+
+def _dptr(t):
+    """Device pointer of a torch CUDA tensor (or a raw int)."""
+    if isinstance(t, int):
+        return C.c_void_p(t)
+    assert t.is_cuda and t.is_contiguous() and t.dtype.is_floating_point and t.element_size() == 8
+    return C.c_void_p(t.data_ptr())
+
+
+def _hptr(a):
+    """Host pointer of a numpy array or a CPU torch tensor (float64, contiguous)."""
+    if isinstance(a, np.ndarray):
+        assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+        return C.c_void_p(a.ctypes.data)
+    assert (not a.is_cuda) and a.is_contiguous() and a.element_size() == 8
+    return C.c_void_p(a.data_ptr())
+
+
+def cm_dg_setup(cfg, stream=None):
+    """cfg: dict with the fields of cm_dg_params (numpy arrays for the HOST pointers).  Returns the ctx handle."""
+    L = _load()
+    p = _Params()
+    p.N = int(cfg["N"])
+    p.ne[:] = [int(v) for v in cfg["ne"]]
+    p.lo[:] = [float(v) for v in cfg["lo"]]
+    p.hi[:] = [float(v) for v in cfg["hi"]]
+    p.bc[:] = [int(v) for v in cfg["bc"]]
+    p.nvar = int(cfg.get("nvar", 5))
+    p.geom = int(cfg.get("geom", 0))
+    keep = []
+
+    def host(key):
+        a = cfg.get(key)
+        if a is None:
+            return None
+        a = np.ascontiguousarray(a, dtype=np.float64)
+        keep.append(a)
+        return C.c_void_p(a.ctypes.data)
+
+    if p.geom == 1:
+        p.zsfc_nodes = host("zsfc_nodes")
+    if p.geom == 2:
+        p.xyz = host("xyz")
+    for k in ("R_d", "c_vd", "R_v", "c_vv", "T_0", "I_v0", "grav", "C_s", "Pr_t", "shf_bottom"):
+        setattr(p, k, float(cfg[k]))
+    p.sgs = int(cfg.get("sgs", 0))
+    p.use_ref = int(cfg.get("use_ref", 0))
+    if p.use_ref:
+        p.ref_rho = host("ref_rho"); p.ref_rhoe = host("ref_rhoe"); p.ref_rhoq = host("ref_rhoq")
+    ctx = C.c_void_p()
+    sp = C.c_void_p(int(stream.cuda_stream)) if stream is not None else C.c_void_p(0)
+    _check(L.cm_dg_setup(C.byref(p), sp, C.byref(ctx)), "cm_dg_setup")
+    return ctx
+
+
+def cm_dg_layout(ctx):
+    L = _load()
+    ne, npn, st = C.c_int64(), C.c_int32(), C.c_int64()
+    _check(L.cm_dg_layout(ctx, C.byref(ne), C.byref(npn), C.byref(st), None), "cm_dg_layout")
+    lex = np.zeros(ne.value, dtype=np.int32)
+    _check(L.cm_dg_layout(ctx, None, None, None, C.c_void_p(lex.ctypes.data)), "cm_dg_layout")
+    return ne.value, npn.value, st.value, lex
+
+
+def cm_dg_coords(ctx, xyz_dev):
+    _check(_load().cm_dg_coords(ctx, _dptr(xyz_dev)), "cm_dg_coords")
+
+
+def cm_dg_metrics(ctx, Ja_dev, J_dev):
+    _check(_load().cm_dg_metrics(ctx, _dptr(Ja_dev), _dptr(J_dev)), "cm_dg_metrics")
+
+
+def cm_dg_gradient(ctx, Q_dev, G_dev):
+    _check(_load().cm_dg_gradient(ctx, _dptr(Q_dev), _dptr(G_dev)), "cm_dg_gradient")
+
+
+def cm_dg_rhs(ctx, Q_dev, dQ_dev, t=0.0):
+    _check(_load().cm_dg_rhs(ctx, _dptr(Q_dev), _dptr(dQ_dev), float(t)), "cm_dg_rhs")
+
+
+def cm_dg_lsrk_step(ctx, Q_dev, t, dt, nsteps):
+    _check(_load().cm_dg_lsrk_step(ctx, _dptr(Q_dev), float(t), float(dt), int(nsteps)), "cm_dg_lsrk_step")
+
+
+def cm_dg_diagnostics(ctx, Q_dev):
+    d = _Diag()
+    _check(_load().cm_dg_diagnostics(ctx, _dptr(Q_dev), C.byref(d)), "cm_dg_diagnostics")
+    return {k: getattr(d, k) for k, _ in _Diag._fields_}
+
+
+def cm_dg_rhs_host(ctx, Q_host, dQ_host, t=0.0):
+    _check(_load().cm_dg_rhs_host(ctx, _hptr(Q_host), _hptr(dQ_host), float(t)), "cm_dg_rhs_host")
+
+
+def cm_dg_lsrk_step_host(ctx, Q_host, t, dt, nsteps):
+    _check(_load().cm_dg_lsrk_step_host(ctx, _hptr(Q_host), float(t), float(dt), int(nsteps)), "cm_dg_lsrk_step_host")
+
+
+def cm_dg_profile_begin(ctx):
+    _check(_load().cm_dg_profile_begin(ctx), "cm_dg_profile_begin")
+
+
+def cm_dg_profile_end(ctx):
+    s = _KStats()
+    _check(_load().cm_dg_profile_end(ctx, C.byref(s)), "cm_dg_profile_end")
+    return {k: getattr(s, k) for k, _ in _KStats._fields_}
+
+
+def cm_dg_destroy(ctx):
+    _load().cm_dg_destroy(ctx)
+
+
+class CmDg:
+    """Owns one ctx; allocates state arrays with torch on the current CUDA device."""
+
+    def __init__(self, cfg, stream=None):
+        import torch
+        self.torch = torch
+        self.cfg = cfg
+        self.ctx = cm_dg_setup(cfg, stream)
+        self.n_elem, self.np, self.stride, self.lex_of_elem = cm_dg_layout(self.ctx)
+        self.nvar = int(cfg.get("nvar", 5))
+        self.device = torch.device("cuda", torch.cuda.current_device())
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            cm_dg_destroy(self.ctx); self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- layout helpers (host side, numpy): lexicographic AoS <-> library SoA
+    def pack(self, Q_lex):
+        """Q_lex[Ne, Np, nv] (lexicographic elements) -> numpy [nv, stride] in library layout."""
+        nv = Q_lex.shape[-1]
+        out = np.zeros((nv, self.stride))
+        out[:, : self.n_elem * self.np] = np.moveaxis(Q_lex[self.lex_of_elem], -1, 0).reshape(nv, -1)
+        return out
+
+    def unpack(self, A):
+        """numpy [nv, stride] in library layout -> [Ne, Np, nv] lexicographic."""
+        nv = A.shape[0]
+        lib = np.moveaxis(A[:, : self.n_elem * self.np].reshape(nv, self.n_elem, self.np), 0, -1)
+        out = np.empty_like(lib)
+        out[self.lex_of_elem] = lib
+        return out
+
+    def to_device(self, Q_lex):
+        return self.torch.from_numpy(self.pack(Q_lex)).to(self.device)
+
+    def to_host(self, T):
+        return self.unpack(T.cpu().numpy())
+
+    def empty(self, nfields):
+        return self.torch.zeros((nfields, self.stride), dtype=self.torch.float64, device=self.device)
+
+    # ---- the C entry points
+    def coords(self):
+        x = self.empty(3); cm_dg_coords(self.ctx, x); return x
+
+    def metrics(self):
+        Ja = self.empty(9); J = self.empty(1); cm_dg_metrics(self.ctx, Ja, J); return Ja, J
+
+    def gradient(self, Q):
+        G = self.empty(15); cm_dg_gradient(self.ctx, Q, G); return G
+
+    def rhs(self, Q, dQ=None, t=0.0):
+        if dQ is None:
+            dQ = self.empty(self.nvar)
+        cm_dg_rhs(self.ctx, Q, dQ, t)
+        return dQ
+
+    def lsrk_step(self, Q, dt, nsteps=1, t=0.0):
+        cm_dg_lsrk_step(self.ctx, Q, t, dt, nsteps)
+        return Q
+
+    def diagnostics(self, Q):
+        return cm_dg_diagnostics(self.ctx, Q)
+
+    def rhs_host(self, Q_host, dQ_host, t=0.0):
+        cm_dg_rhs_host(self.ctx, Q_host, dQ_host, t)
+
+    def lsrk_step_host(self, Q_host, dt, nsteps=1, t=0.0):
+        cm_dg_lsrk_step_host(self.ctx, Q_host, t, dt, nsteps)
+
+    def profile_begin(self):
+        cm_dg_profile_begin(self.ctx)
+
+    def profile_end(self):
+        return cm_dg_profile_end(self.ctx)

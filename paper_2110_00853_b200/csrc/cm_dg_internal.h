@@ -1,0 +1,63 @@
+// cm_dg_internal.h -- shared declarations of the CUDA implementation behind include/cm_dg.h.
+// Not part of the public boundary.  P:L<n> = line of the paper text.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#define CM_MAXNQ 8
+#define CM_ZTAB_W 8   // doubles per z-table row (flat meshes): Phi, rho_r, rhoe_r, rhoq_r, E_r, q_r, 1/c_vm_r, unused
+#define CM_NGEO 12    // general geometry, per node: Ja[9], 1/J, z, (C_s Delta)^2
+
+// Thermodynamic constants of eq. (7)-(14) in the combinations the kernels use.
+struct CmThermo {
+  double R_d, c_vd;
+  double a;    // R_v - R_d
+  double b;    // c_vv - c_vd
+  double T_0, I_v0, grav;
+  double dk;   // a c_vd - R_d b   (numerator of kappa - kappa_r, reading R12)
+};
+
+// Kernel argument block (passed by value, lives in the constant bank).
+struct CmKP {
+  // sizes
+  int Ne;                // elements
+  long long stride;      // field stride in doubles
+  int sgs;               // Smagorinsky-Lilly on/off
+  int use_ref;           // reference state removed (R12) or plain pressure
+  int mode;              // tendency: 0 dQ := rhs | 1 LSRK stage.  gradient: 0 packed SGS fluxes | 1 raw 15 gradients
+  // arrays
+  const double* Q;       // [nvar][stride]
+  const double* G;       // packed SGS fluxes [ngrad][stride] (tendency input)
+  double* Gout;          // gradient output
+  double* dQ;            // residual (in/out) or rhs output
+  double* Qnew;          // LSRK: updated state (ping-pong buffer)
+  const int* nbr;        // [Ne][6] neighbour in library order, <0 = wall
+  const int* erow;       // flat: [Ne] first z-table row of the element (= ez*Nq)
+  const double* ztab;    // flat: [Ez*Nq][CM_ZTAB_W]
+  const double* geo;     // general: [CM_NGEO][stride]
+  const double* ref;     // general: [3][stride] rho_r, rhoe_r, rhoq_r
+  // constants
+  CmThermo th;
+  double cA[3];          // flat: Ja^d_d = h_e h_f / 4
+  double invJ;           // flat: 8 / (hx hy hz)
+  double cs2delta2;      // flat: (C_s Delta)^2
+  double inv_Pr;
+  double shf;            // prescribed upward energy flux at the bottom wall
+  double inv_w0;         // 1 / w_0 = N (N+1) / 2
+  double rka, rkb, dt;   // LSRK stage coefficients
+  double D[CM_MAXNQ][CM_MAXNQ];  // D[i][m] = L_m'(xi_i)
+};
+
+struct CmLaunchCfg { int epb; int threads; size_t smem_grad; size_t smem_tend; };
+
+// implemented in cm_dg_kernels_inst.cu (one object per polynomial order)
+typedef cudaError_t (*cm_launch_fn)(const CmKP& kp, int moist, int general, cudaStream_t st);
+#define CM_DECL_LAUNCHERS(NQ)                                                                 \
+  cudaError_t cm_launch_gradient_nq##NQ(const CmKP& kp, int moist, int general, cudaStream_t st); \
+  cudaError_t cm_launch_tendency_nq##NQ(const CmKP& kp, int moist, int general, cudaStream_t st);
+CM_DECL_LAUNCHERS(3)
+CM_DECL_LAUNCHERS(4)
+CM_DECL_LAUNCHERS(5)
+CM_DECL_LAUNCHERS(6)
+CM_DECL_LAUNCHERS(7)
+CM_DECL_LAUNCHERS(8)

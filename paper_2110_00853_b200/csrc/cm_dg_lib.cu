@@ -1,0 +1,712 @@
+// cm_dg_lib.cu -- host side of the C ABI in include/cm_dg.h plus the setup / diagnostics kernels:
+//   a0  LGL nodes, weights, derivative matrix; element ordering and connectivity; metric terms
+//       (eq. 24) by a CUDA kernel; reference-state tables
+//   a6  conservation integrals (eq. 57, 61, 62)
+// The hot kernels live in cm_dg_kernels.cuh.  There is no CPU fallback anywhere in this file: every
+// entry point that computes needs a CUDA device and fails with CM_DG_ECUDA without one.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/cm_dg.h"
+#include "cm_dg_internal.h"
+
+namespace {
+
+thread_local std::string g_err = "";
+int fail(int code, const std::string& msg) { g_err = msg; return code; }
+#define CM_CUDA(call)                                                                                    \
+  do {                                                                                                   \
+    cudaError_t err__ = (call);                                                                          \
+    if (err__ != cudaSuccess)                                                                            \
+      return fail(err__ == cudaErrorMemoryAllocation ? CM_DG_ENOMEM : CM_DG_ECUDA,                       \
+                  std::string(#call) + ": " + cudaGetErrorString(err__));                                \
+  } while (0)
+
+// LSRK54 of Carpenter & Kennedy (1994), 2N-storage (5,4) scheme (P:L286 cites the family).
+const double kRKA[5] = {0.0, -567301805773.0 / 1357537059087.0, -2404267990393.0 / 2016746695238.0,
+                        -3550918686646.0 / 2091501179385.0, -1275806237668.0 / 842570457699.0};
+const double kRKB[5] = {1432997174477.0 / 9575080441755.0, 5161836677717.0 / 13612068292357.0,
+                        1720146321549.0 / 2090206949498.0, 3134564353537.0 / 4481467310338.0,
+                        2277821191437.0 / 14882151754819.0};
+
+// ------------------------------------------------------------------ a0: 1-D operators
+// LGL points as the roots of q(x) = P_{N+1}(x) - P_{N-1}(x) (proportional to (1 - x^2) P_N'(x)), Newton in
+// long double; weights 2 / (N (N+1) P_N^2); D from barycentric weights with the negative-sum diagonal.
+void lgl_operators(int N, double* xi, double* w, double (*D)[CM_MAXNQ]) {
+  const int Nq = N + 1;
+  std::vector<long double> x(Nq);
+  const long double pi = 3.14159265358979323846264338327950288L;
+  auto legendre3 = [&](long double t, long double& Pm1, long double& P0, long double& Pp1) {
+    long double a = 1.0L, b = t;   // P_0, P_1
+    for (int n = 1; n < N; ++n) { long double c = ((2 * n + 1) * t * b - n * a) / (n + 1); a = b; b = c; }
+    // now a = P_{N-1}, b = P_N
+    Pm1 = a; P0 = b; Pp1 = ((2 * N + 1) * t * b - N * a) / (N + 1);
+  };
+  for (int i = 0; i < Nq; ++i) {
+    long double t = -std::cos(pi * i / N);
+    if (i == 0) t = -1.0L; else if (i == N) t = 1.0L;
+    else
+      for (int it = 0; it < 60; ++it) {
+        long double a, b, c; legendre3(t, a, b, c);
+        long double q = c - a, dq = (2 * N + 1) * b;          // q' = (2N+1) P_N
+        long double dt = q / dq; t -= dt;
+        if (fabsl(dt) < 1e-20L) break;
+      }
+    x[i] = t;
+  }
+  for (int i = 0; i < Nq / 2; ++i) { long double m = 0.5L * (x[N - i] - x[i]); x[i] = -m; x[N - i] = m; }
+  if (N % 2 == 0) x[N / 2] = 0.0L;
+  std::vector<long double> bw(Nq);
+  for (int i = 0; i < Nq; ++i) {
+    long double a, b, c; legendre3(x[i], a, b, c);
+    xi[i] = (double)x[i];
+    w[i] = (double)(2.0L / (N * (N + 1.0L) * b * b));
+    long double prod = 1.0L;
+    for (int l = 0; l < Nq; ++l) if (l != i) prod *= (x[i] - x[l]);
+    bw[i] = 1.0L / prod;
+  }
+  for (int i = 0; i < Nq; ++i) {
+    long double s = 0.0L;
+    for (int j = 0; j < Nq; ++j) {
+      if (i == j) continue;
+      long double dij = (bw[j] / bw[i]) / (x[i] - x[j]);
+      D[i][j] = (double)dij; s += dij;
+    }
+    D[i][i] = (double)(-s);
+  }
+}
+
+// ------------------------------------------------------------------ small kernels
+struct GeoArgs {
+  int Nq, Np, geom;
+  long long Ne, stride;
+  int ne[3];
+  double lo[3], hi[3], h[3];
+  const int* lex;         // [Ne] lexicographic id of library element
+  const double* zsfc;     // geom 1
+  const double* xyz_user; // geom 2: [3][stride] library order
+  double xi[CM_MAXNQ], w[CM_MAXNQ], D[CM_MAXNQ][CM_MAXNQ];
+  double cs, grav;
+};
+
+__device__ inline void node_xyz(const GeoArgs& a, long long e, int n, double* X) {
+  if (a.geom == 2) {
+    for (int d = 0; d < 3; ++d) X[d] = a.xyz_user[d * a.stride + e * a.Np + n];
+    return;
+  }
+  const int lex = a.lex[e];
+  const int ec[3] = {lex % a.ne[0], (lex / a.ne[0]) % a.ne[1], lex / (a.ne[0] * a.ne[1])};
+  const int ijk[3] = {n % a.Nq, (n / a.Nq) % a.Nq, n / (a.Nq * a.Nq)};
+  for (int d = 0; d < 3; ++d) X[d] = a.lo[d] + (ec[d] + 0.5 * (a.xi[ijk[d]] + 1.0)) * a.h[d];
+  if (a.geom == 1) {
+    const double zs = a.zsfc[(long long)(ec[1] * a.Nq + ijk[1]) * (a.ne[0] * a.Nq) + ec[0] * a.Nq + ijk[0]];
+    X[2] += zs * (a.hi[2] - X[2]) / (a.hi[2] - a.lo[2]);      // linear decay to a flat lid
+  }
+}
+
+__global__ void coords_kernel(const __grid_constant__ GeoArgs a, double* __restrict__ xyz) {
+  const long long e = blockIdx.x;
+  for (int n = threadIdx.x; n < a.Np; n += blockDim.x) {
+    double X[3]; node_xyz(a, e, n, X);
+    for (int d = 0; d < 3; ++d) xyz[d * a.stride + e * a.Np + n] = X[d];
+  }
+}
+
+// metric terms of one element per block: geo = Ja[9], 1/J, z, (C_s Delta)^2; chk[e] = {min J, metric-identity
+// residual / max|Ja|, min node spacing}
+__global__ void metrics_kernel(const __grid_constant__ GeoArgs a, double* __restrict__ geo, double* __restrict__ chk) {
+  extern __shared__ double sh[];
+  double* X = sh;                 // [3][Np]
+  double* JA = sh + 3 * a.Np;     // [9][Np]
+  double* red = JA + 9 * a.Np;    // [3][blockDim]
+  const long long e = blockIdx.x;
+  const int Nq = a.Nq, Np = a.Np;
+  for (int n = threadIdx.x; n < Np; n += blockDim.x) {
+    double P[3]; node_xyz(a, e, n, P);
+    for (int d = 0; d < 3; ++d) X[d * Np + n] = P[d];
+  }
+  __syncthreads();
+  double minJ = 1e300, mindx = 1e300, amax = 0.0;
+  for (int n = threadIdx.x; n < Np; n += blockDim.x) {
+    const int i = n % Nq, j = (n / Nq) % Nq, k = n / (Nq * Nq);
+    double xr[3] = {0, 0, 0}, xs[3] = {0, 0, 0}, xt[3] = {0, 0, 0};
+    for (int m = 0; m < Nq; ++m)
+      for (int d = 0; d < 3; ++d) {
+        xr[d] += a.D[i][m] * X[d * Np + m + Nq * (j + Nq * k)];
+        xs[d] += a.D[j][m] * X[d * Np + i + Nq * (m + Nq * k)];
+        xt[d] += a.D[k][m] * X[d * Np + i + Nq * (j + Nq * m)];
+      }
+    double A[9];
+    A[0] = xs[1] * xt[2] - xs[2] * xt[1]; A[1] = xs[2] * xt[0] - xs[0] * xt[2]; A[2] = xs[0] * xt[1] - xs[1] * xt[0];
+    A[3] = xt[1] * xr[2] - xt[2] * xr[1]; A[4] = xt[2] * xr[0] - xt[0] * xr[2]; A[5] = xt[0] * xr[1] - xt[1] * xr[0];
+    A[6] = xr[1] * xs[2] - xr[2] * xs[1]; A[7] = xr[2] * xs[0] - xr[0] * xs[2]; A[8] = xr[0] * xs[1] - xr[1] * xs[0];
+    const double J = xr[0] * A[0] + xr[1] * A[1] + xr[2] * A[2];
+    const long long idx = e * Np + n;
+    for (int m = 0; m < 9; ++m) { geo[m * a.stride + idx] = A[m]; JA[m * Np + n] = A[m]; amax = fmax(amax, fabs(A[m])); }
+    geo[9 * a.stride + idx] = 1.0 / J;
+    geo[10 * a.stride + idx] = X[2 * Np + n];
+    const double delta = cbrt(8.0 * J) / (Nq - 1);              // filter width, reading R7
+    geo[11 * a.stride + idx] = (a.cs * delta) * (a.cs * delta);
+    minJ = fmin(minJ, J);
+    const int nb[3] = {(i + 1 < Nq) ? n + 1 : -1, (j + 1 < Nq) ? n + Nq : -1, (k + 1 < Nq) ? n + Nq * Nq : -1};
+    for (int d = 0; d < 3; ++d)
+      if (nb[d] >= 0) {
+        double s = 0;
+        for (int c = 0; c < 3; ++c) { const double t = X[c * Np + nb[d]] - X[c * Np + n]; s += t * t; }
+        mindx = fmin(mindx, sqrt(s));
+      }
+  }
+  __syncthreads();
+  double res = 0.0;
+  for (int n = threadIdx.x; n < Np; n += blockDim.x) {
+    const int i = n % Nq, j = (n / Nq) % Nq, k = n / (Nq * Nq);
+    for (int c = 0; c < 3; ++c) {
+      double r = 0.0;
+      for (int m = 0; m < Nq; ++m)
+        r += a.D[i][m] * JA[(0 + c) * Np + m + Nq * (j + Nq * k)] + a.D[j][m] * JA[(3 + c) * Np + i + Nq * (m + Nq * k)] +
+             a.D[k][m] * JA[(6 + c) * Np + i + Nq * (j + Nq * m)];
+      res = fmax(res, fabs(r));
+    }
+  }
+  red[threadIdx.x] = minJ; red[blockDim.x + threadIdx.x] = res; red[2 * blockDim.x + threadIdx.x] = mindx;
+  double* red4 = red + 3 * blockDim.x; red4[threadIdx.x] = amax;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double mj = 1e300, rr = 0, md = 1e300, am = 0;
+    for (int t = 0; t < blockDim.x; ++t) {
+      mj = fmin(mj, red[t]); rr = fmax(rr, red[blockDim.x + t]); md = fmin(md, red[2 * blockDim.x + t]); am = fmax(am, red4[t]);
+    }
+    chk[3 * e] = mj; chk[3 * e + 1] = rr / fmax(am, 1e-300); chk[3 * e + 2] = md;
+  }
+}
+
+__global__ void flat_metrics_fill(long long n, long long stride, const double cA0, const double cA1, const double cA2,
+                                  const double J, double* __restrict__ Ja, double* __restrict__ Jout) {
+  const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  for (int m = 0; m < 9; ++m) Ja[m * stride + t] = 0.0;
+  Ja[0 * stride + t] = cA0; Ja[4 * stride + t] = cA1; Ja[8 * stride + t] = cA2;
+  Jout[t] = J;
+}
+
+__global__ void general_metrics_copy(long long n, long long stride, const double* __restrict__ geo,
+                                     double* __restrict__ Ja, double* __restrict__ Jout) {
+  const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  for (int m = 0; m < 9; ++m) Ja[m * stride + t] = geo[m * stride + t];
+  Jout[t] = 1.0 / geo[9 * stride + t];
+}
+
+// a6: per-block partial sums {mass, energy, water, M |u|^2 / 2, M, max(|u|+c), nonfinite}
+struct DiagArgs {
+  int Nq, Np, nvar, general, use_ref;
+  long long Ne, stride;
+  const double* Q; const double* geo; const int* erow; const double* ztab;
+  double Jflat; double w[CM_MAXNQ];
+  CmThermo th;
+};
+
+__global__ void diag_kernel(const __grid_constant__ DiagArgs a, double* __restrict__ part) {
+  extern __shared__ double sh[];
+  const long long e = blockIdx.x;
+  double s[7] = {0, 0, 0, 0, 0, 0, 0};
+  for (int n = threadIdx.x; n < a.Np; n += blockDim.x) {
+    const int i = n % a.Nq, j = (n / a.Nq) % a.Nq, k = n / (a.Nq * a.Nq);
+    const long long idx = e * a.Np + n;
+    double Y[6] = {0, 0, 0, 0, 0, 0};
+    for (int v = 0; v < a.nvar; ++v) { Y[v] = a.Q[v * a.stride + idx]; if (!isfinite(Y[v])) s[6] += 1.0; }
+    const double J = a.general ? 1.0 / a.geo[9 * a.stride + idx] : a.Jflat;
+    const double Phi = a.general ? a.th.grav * a.geo[10 * a.stride + idx] : a.ztab[(long long)(a.erow[e] + k) * CM_ZTAB_W];
+    const double M = a.w[i] * a.w[j] * a.w[k] * J;
+    const double ir = 1.0 / Y[0];
+    const double u2 = (Y[1] * Y[1] + Y[2] * Y[2] + Y[3] * Y[3]) * ir * ir;
+    const double q = (a.nvar == 6) ? Y[5] * ir : 0.0;
+    const double cvm = a.th.c_vd + a.th.b * q, Rm = a.th.R_d + a.th.a * q;
+    const double eint = Y[4] * ir - 0.5 * u2 - Phi;
+    const double T = a.th.T_0 + (eint - q * a.th.I_v0) / cvm;
+    const double c = sqrt((1.0 + Rm / cvm) * Rm * T);
+    s[0] += M * Y[0]; s[1] += M * Y[4]; s[2] += M * Y[5]; s[3] += M * 0.5 * u2; s[4] += M;
+    s[5] = fmax(s[5], sqrt(u2) + c);
+  }
+  for (int m = 0; m < 7; ++m) sh[m * blockDim.x + threadIdx.x] = s[m];
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double r[7] = {0, 0, 0, 0, 0, 0, 0};
+    for (int t = 0; t < blockDim.x; ++t)
+      for (int m = 0; m < 7; ++m) r[m] = (m == 5) ? fmax(r[m], sh[m * blockDim.x + t]) : r[m] + sh[m * blockDim.x + t];
+    for (int m = 0; m < 7; ++m) part[7 * e + m] = r[m];
+  }
+}
+
+// ------------------------------------------------------------------ element ordering
+// Library order: elements grouped in T x T x T tiles (x fastest inside a tile), tiles along a Morton curve,
+// so that the six face neighbours of an element are mostly a few KB..MB away (L2-resident traces).
+inline uint64_t spread3(uint64_t v) {
+  uint64_t r = 0;
+  for (int b = 0; b < 21; ++b) r |= ((v >> b) & 1ull) << (3 * b);
+  return r;
+}
+
+}  // namespace
+
+struct cm_dg_ctx {
+  cm_dg_params prm;
+  int N, Nq, Np, nvar, ngrad, general, moist;
+  int64_t Ne, stride;
+  cudaStream_t st;
+  std::vector<int32_t> lex_of_elem;
+  double xi[CM_MAXNQ], w[CM_MAXNQ], D[CM_MAXNQ][CM_MAXNQ];
+  double h[3], min_node_dx;
+  // device
+  int *d_nbr = nullptr, *d_erow = nullptr, *d_lex = nullptr;
+  double *d_ztab = nullptr, *d_geo = nullptr, *d_ref = nullptr, *d_G = nullptr, *d_res = nullptr, *d_Q2 = nullptr;
+  double *d_zsfc = nullptr, *d_xyz_user = nullptr, *d_part = nullptr, *d_stage = nullptr;
+  CmKP kp;
+  cm_launch_fn launch_grad = nullptr, launch_tend = nullptr;
+  // profiling
+  bool profiling = false;
+  std::vector<cudaEvent_t> ev;   // pairs (start, stop)
+  std::vector<int> ev_kind;      // per pair: 0 gradient, 1 tendency, 2 other
+  size_t ev_used = 0;
+};
+
+namespace {
+
+void free_ctx(cm_dg_ctx* c) {
+  if (!c) return;
+  cudaFree(c->d_nbr); cudaFree(c->d_erow); cudaFree(c->d_lex); cudaFree(c->d_ztab); cudaFree(c->d_geo);
+  cudaFree(c->d_ref); cudaFree(c->d_G); cudaFree(c->d_res); cudaFree(c->d_Q2); cudaFree(c->d_zsfc);
+  cudaFree(c->d_xyz_user); cudaFree(c->d_part); cudaFree(c->d_stage);
+  for (auto e : c->ev) cudaEventDestroy(e);
+  delete c;
+}
+
+GeoArgs geo_args(const cm_dg_ctx* c) {
+  GeoArgs a;
+  a.Nq = c->Nq; a.Np = c->Np; a.geom = c->prm.geom; a.Ne = c->Ne; a.stride = c->stride;
+  for (int d = 0; d < 3; ++d) { a.ne[d] = c->prm.ne[d]; a.lo[d] = c->prm.lo[d]; a.hi[d] = c->prm.hi[d]; a.h[d] = c->h[d]; }
+  a.lex = c->d_lex; a.zsfc = c->d_zsfc; a.xyz_user = c->d_xyz_user;
+  for (int i = 0; i < CM_MAXNQ; ++i) { a.xi[i] = c->xi[i]; a.w[i] = c->w[i]; for (int j = 0; j < CM_MAXNQ; ++j) a.D[i][j] = c->D[i][j]; }
+  a.cs = c->prm.C_s; a.grav = c->prm.grav;
+  return a;
+}
+
+// timed launch helper
+struct Timed {
+  cm_dg_ctx* c; int kind; bool on;
+  Timed(cm_dg_ctx* c_, int kind_) : c(c_), kind(kind_), on(c_->profiling) {
+    if (!on) return;
+    if (c->ev_used + 2 > c->ev.size()) {
+      for (int t = 0; t < 2; ++t) { cudaEvent_t e; cudaEventCreate(&e); c->ev.push_back(e); }
+      c->ev_kind.push_back(kind);
+    }
+    c->ev_kind[c->ev_used / 2] = kind;
+    cudaEventRecord(c->ev[c->ev_used], c->st);
+  }
+  ~Timed() {
+    if (!on) return;
+    cudaEventRecord(c->ev[c->ev_used + 1], c->st);
+    c->ev_used += 2;
+  }
+};
+
+int run_gradient(cm_dg_ctx* c, const double* Q, double* Gout, int raw) {
+  CmKP kp = c->kp;
+  kp.Q = Q; kp.Gout = Gout; kp.mode = raw;
+  Timed t(c, 0);
+  cudaError_t err = c->launch_grad(kp, c->moist, c->general, c->st);
+  if (err != cudaSuccess) return fail(CM_DG_ECUDA, std::string("gradient kernel launch: ") + cudaGetErrorString(err));
+  return CM_DG_OK;
+}
+
+int run_tendency(cm_dg_ctx* c, const double* Q, double* dQ, double* Qnew, int mode, double rka, double rkb, double dt) {
+  CmKP kp = c->kp;
+  kp.Q = Q; kp.G = c->d_G; kp.dQ = dQ; kp.Qnew = Qnew; kp.mode = mode; kp.rka = rka; kp.rkb = rkb; kp.dt = dt;
+  Timed t(c, 1);
+  cudaError_t err = c->launch_tend(kp, c->moist, c->general, c->st);
+  if (err != cudaSuccess) return fail(CM_DG_ECUDA, std::string("tendency kernel launch: ") + cudaGetErrorString(err));
+  return CM_DG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* cm_dg_last_error(void) { return g_err.c_str(); }
+
+void cm_dg_destroy(cm_dg_ctx* ctx) { free_ctx(ctx); }
+
+int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
+  if (!p || !out) return fail(CM_DG_EINVAL, "cm_dg_setup: NULL argument");
+  *out = nullptr;
+  if (p->N < 2 || p->N > 7) return fail(CM_DG_EINVAL, "cm_dg_setup: polynomial order N must be in 2..7");
+  if (p->nvar != 5 && p->nvar != 6) return fail(CM_DG_EINVAL, "cm_dg_setup: nvar must be 5 or 6");
+  for (int d = 0; d < 3; ++d) {
+    if (p->ne[d] < 1) return fail(CM_DG_EINVAL, "cm_dg_setup: ne[d] must be >= 1");
+    if (!(p->hi[d] > p->lo[d])) return fail(CM_DG_EINVAL, "cm_dg_setup: hi[d] must exceed lo[d]");
+    if (p->bc[d] != 0 && p->bc[d] != 1) return fail(CM_DG_EINVAL, "cm_dg_setup: bc[d] must be 0 (periodic) or 1 (wall)");
+  }
+  if (p->geom < 0 || p->geom > 2) return fail(CM_DG_EINVAL, "cm_dg_setup: geom must be 0, 1 or 2");
+  if (p->geom == 1 && !p->zsfc_nodes) return fail(CM_DG_EINVAL, "cm_dg_setup: geom == 1 needs zsfc_nodes");
+  if (p->geom == 2 && !p->xyz) return fail(CM_DG_EINVAL, "cm_dg_setup: geom == 2 needs xyz");
+  if (p->use_ref && (!p->ref_rho || !p->ref_rhoe || (p->nvar == 6 && !p->ref_rhoq)))
+    return fail(CM_DG_EINVAL, "cm_dg_setup: use_ref needs ref_rho, ref_rhoe (and ref_rhoq when nvar == 6)");
+  if (p->sgs && !(p->Pr_t > 0.0)) return fail(CM_DG_EINVAL, "cm_dg_setup: Pr_t must be positive");
+  if (!(p->c_vd > 0.0) || !(p->R_d > 0.0)) return fail(CM_DG_EINVAL, "cm_dg_setup: R_d and c_vd must be positive");
+  const int64_t Ne = (int64_t)p->ne[0] * p->ne[1] * p->ne[2];
+  const int Nq = p->N + 1, Np = Nq * Nq * Nq;
+  if (Ne * Np >= (int64_t)1 << 31) return fail(CM_DG_EINVAL, "cm_dg_setup: more than 2^31 nodes");
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+    return fail(CM_DG_ECUDA, "cm_dg_setup: no CUDA device (this library has no CPU path)");
+
+  cm_dg_ctx* c = new cm_dg_ctx();
+  c->prm = *p;
+  c->prm.zsfc_nodes = nullptr; c->prm.xyz = nullptr; c->prm.ref_rho = c->prm.ref_rhoe = c->prm.ref_rhoq = nullptr;
+  c->N = p->N; c->Nq = Nq; c->Np = Np; c->nvar = p->nvar; c->moist = (p->nvar == 6);
+  c->ngrad = c->moist ? 12 : 9;
+  c->Ne = Ne;
+  c->stride = ((Ne * Np + 31) / 32) * 32;
+  c->st = (cudaStream_t)cuda_stream;
+  for (int d = 0; d < 3; ++d) c->h[d] = (p->hi[d] - p->lo[d]) / p->ne[d];
+  std::memset(c->D, 0, sizeof(c->D));
+  lgl_operators(c->N, c->xi, c->w, c->D);
+
+  // ---- element order
+  {
+    const char* ord = std::getenv("CM_DG_ORDER");
+    const bool lex_order = ord && std::strcmp(ord, "lex") == 0;
+    const int T = 4;
+    std::vector<std::pair<uint64_t, int32_t>> keys(Ne);
+    for (int64_t l = 0; l < Ne; ++l) {
+      const int ex = (int)(l % p->ne[0]), ey = (int)((l / p->ne[0]) % p->ne[1]), ez = (int)(l / ((int64_t)p->ne[0] * p->ne[1]));
+      uint64_t key;
+      if (lex_order) key = (uint64_t)l;
+      else {
+        const uint64_t tile = spread3(ex / T) | (spread3(ey / T) << 1) | (spread3(ez / T) << 2);
+        const uint64_t local = (uint64_t)((ex % T) + T * ((ey % T) + T * (ez % T)));
+        key = (tile << 6) | local;
+      }
+      keys[l] = {key, (int32_t)l};
+    }
+    std::sort(keys.begin(), keys.end());
+    c->lex_of_elem.resize(Ne);
+    for (int64_t e = 0; e < Ne; ++e) c->lex_of_elem[e] = keys[e].second;
+  }
+  std::vector<int32_t> pos_of_lex(Ne);
+  for (int64_t e = 0; e < Ne; ++e) pos_of_lex[c->lex_of_elem[e]] = (int32_t)e;
+
+  // ---- connectivity: faces 0..5 = -xi, +xi, -eta, +eta, -zeta, +zeta; -1 = wall
+  std::vector<int32_t> nbr(Ne * 6), erow(Ne);
+  for (int64_t e = 0; e < Ne; ++e) {
+    const int64_t l = c->lex_of_elem[e];
+    int ec[3] = {(int)(l % p->ne[0]), (int)((l / p->ne[0]) % p->ne[1]), (int)(l / ((int64_t)p->ne[0] * p->ne[1]))};
+    erow[e] = ec[2] * Nq;
+    for (int f = 0; f < 6; ++f) {
+      const int d = f / 2;
+      int v[3] = {ec[0], ec[1], ec[2]};
+      v[d] += (f % 2) ? 1 : -1;
+      if (v[d] < 0 || v[d] >= p->ne[d]) {
+        if (p->bc[d] == 1) { nbr[e * 6 + f] = -1; continue; }
+        v[d] = (v[d] + p->ne[d]) % p->ne[d];
+      }
+      nbr[e * 6 + f] = pos_of_lex[v[0] + (int64_t)p->ne[0] * (v[1] + (int64_t)p->ne[1] * v[2])];
+    }
+  }
+
+  // ---- reference state: z-only table on flat meshes, per-node arrays otherwise
+  const size_t nn = (size_t)Ne * Np;
+  bool ref_z_only = true;
+  if (p->use_ref && p->geom == 0) {
+    const int64_t nh = (int64_t)p->ne[0] * p->ne[1];
+    for (int ez = 0; ez < p->ne[2] && ref_z_only; ++ez)
+      for (int k = 0; k < Nq && ref_z_only; ++k) {
+        const size_t first = ((size_t)ez * nh) * Np + (size_t)k * Nq * Nq;
+        for (int64_t hh = 0; hh < nh && ref_z_only; ++hh)
+          for (int m = 0; m < Nq * Nq; ++m) {
+            const size_t id = ((size_t)ez * nh + hh) * Np + (size_t)k * Nq * Nq + m;
+            if (p->ref_rho[id] != p->ref_rho[first] || p->ref_rhoe[id] != p->ref_rhoe[first] ||
+                (c->moist && p->ref_rhoq[id] != p->ref_rhoq[first])) { ref_z_only = false; break; }
+          }
+      }
+  }
+  c->general = (p->geom != 0 || (p->use_ref && !ref_z_only)) ? 1 : 0;
+  if (const char* fg = std::getenv("CM_DG_FORCE_GENERAL")) if (fg[0] == '1') c->general = 1;
+
+  auto bail = [&](int code) { free_ctx(c); return code; };
+#define CM_CUDA_B(call)                                                                                   \
+  do {                                                                                                    \
+    cudaError_t err__ = (call);                                                                           \
+    if (err__ != cudaSuccess) {                                                                           \
+      fail(err__ == cudaErrorMemoryAllocation ? CM_DG_ENOMEM : CM_DG_ECUDA, std::string(#call) + ": " + cudaGetErrorString(err__)); \
+      return bail(err__ == cudaErrorMemoryAllocation ? CM_DG_ENOMEM : CM_DG_ECUDA);                       \
+    }                                                                                                     \
+  } while (0)
+
+  const size_t fbytes = (size_t)c->stride * sizeof(double);
+  CM_CUDA_B(cudaMalloc(&c->d_nbr, nbr.size() * sizeof(int32_t)));
+  CM_CUDA_B(cudaMalloc(&c->d_erow, erow.size() * sizeof(int32_t)));
+  CM_CUDA_B(cudaMalloc(&c->d_lex, (size_t)Ne * sizeof(int32_t)));
+  CM_CUDA_B(cudaMemcpy(c->d_nbr, nbr.data(), nbr.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+  CM_CUDA_B(cudaMemcpy(c->d_erow, erow.data(), erow.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+  CM_CUDA_B(cudaMemcpy(c->d_lex, c->lex_of_elem.data(), (size_t)Ne * sizeof(int32_t), cudaMemcpyHostToDevice));
+  if (p->geom == 1) {
+    const size_t nz = (size_t)p->ne[0] * Nq * p->ne[1] * Nq;
+    CM_CUDA_B(cudaMalloc(&c->d_zsfc, nz * sizeof(double)));
+    CM_CUDA_B(cudaMemcpy(c->d_zsfc, p->zsfc_nodes, nz * sizeof(double), cudaMemcpyHostToDevice));
+  }
+  if (p->geom == 2) {
+    std::vector<double> tmp((size_t)3 * c->stride, 0.0);
+    for (int d = 0; d < 3; ++d)
+      for (int64_t e = 0; e < Ne; ++e)
+        std::memcpy(&tmp[(size_t)d * c->stride + (size_t)e * Np], p->xyz + ((size_t)d * Ne + c->lex_of_elem[e]) * Np, Np * sizeof(double));
+    CM_CUDA_B(cudaMalloc(&c->d_xyz_user, tmp.size() * sizeof(double)));
+    CM_CUDA_B(cudaMemcpy(c->d_xyz_user, tmp.data(), tmp.size() * sizeof(double), cudaMemcpyHostToDevice));
+  }
+
+  // ---- kernel parameter block
+  CmKP& kp = c->kp;
+  std::memset(&kp, 0, sizeof(kp));
+  kp.Ne = (int)Ne; kp.stride = c->stride; kp.sgs = p->sgs ? 1 : 0; kp.use_ref = p->use_ref ? 1 : 0;
+  kp.th.R_d = p->R_d; kp.th.c_vd = p->c_vd; kp.th.a = p->R_v - p->R_d; kp.th.b = p->c_vv - p->c_vd;
+  kp.th.T_0 = p->T_0; kp.th.I_v0 = p->I_v0; kp.th.grav = p->grav;
+  kp.th.dk = kp.th.a * p->c_vd - p->R_d * kp.th.b;
+  kp.cA[0] = c->h[1] * c->h[2] / 4.0; kp.cA[1] = c->h[0] * c->h[2] / 4.0; kp.cA[2] = c->h[0] * c->h[1] / 4.0;
+  kp.invJ = 8.0 / (c->h[0] * c->h[1] * c->h[2]);
+  {
+    const double delta = std::cbrt(c->h[0] * c->h[1] * c->h[2]) / c->N;
+    kp.cs2delta2 = (p->C_s * delta) * (p->C_s * delta);
+  }
+  kp.inv_Pr = p->sgs ? 1.0 / p->Pr_t : 0.0;
+  kp.shf = p->shf_bottom;
+  kp.inv_w0 = 1.0 / c->w[0];
+  for (int i = 0; i < CM_MAXNQ; ++i) for (int j = 0; j < CM_MAXNQ; ++j) kp.D[i][j] = c->D[i][j];
+  kp.nbr = c->d_nbr; kp.erow = c->d_erow;
+
+  c->min_node_dx = std::min(c->h[0], std::min(c->h[1], c->h[2])) * 0.5 * (c->xi[1] - c->xi[0]);
+
+  if (!c->general) {
+    // z table: Phi and the reference column per (ez, k)
+    const int rows = p->ne[2] * Nq;
+    std::vector<double> zt((size_t)rows * CM_ZTAB_W, 0.0);
+    const int64_t nh = (int64_t)p->ne[0] * p->ne[1];
+    for (int ez = 0; ez < p->ne[2]; ++ez)
+      for (int k = 0; k < Nq; ++k) {
+        double* t = &zt[(size_t)(ez * Nq + k) * CM_ZTAB_W];
+        const double z = p->lo[2] + (ez + 0.5 * (c->xi[k] + 1.0)) * c->h[2];
+        t[0] = p->grav * z;
+        if (p->use_ref) {
+          const size_t id = ((size_t)ez * nh) * Np + (size_t)k * Nq * Nq;
+          t[1] = p->ref_rho[id]; t[2] = p->ref_rhoe[id]; t[3] = c->moist ? p->ref_rhoq[id] : 0.0;
+          t[4] = t[2] - t[1] * t[0] - t[3] * p->I_v0;
+          t[5] = t[3] / t[1];
+          t[6] = 1.0 / (p->c_vd + kp.th.b * t[5]);
+        }
+      }
+    CM_CUDA_B(cudaMalloc(&c->d_ztab, zt.size() * sizeof(double)));
+    CM_CUDA_B(cudaMemcpy(c->d_ztab, zt.data(), zt.size() * sizeof(double), cudaMemcpyHostToDevice));
+    kp.ztab = c->d_ztab;
+  } else {
+    CM_CUDA_B(cudaMalloc(&c->d_geo, (size_t)CM_NGEO * fbytes));
+    CM_CUDA_B(cudaMemset(c->d_geo, 0, (size_t)CM_NGEO * fbytes));
+    double* d_chk = nullptr;
+    CM_CUDA_B(cudaMalloc(&d_chk, (size_t)Ne * 3 * sizeof(double)));
+    GeoArgs ga = geo_args(c);
+    const int thr = 128;
+    const size_t sm = (size_t)(12 * Np + 4 * thr) * sizeof(double);
+    cudaFuncSetAttribute(metrics_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    metrics_kernel<<<(unsigned)Ne, thr, sm, c->st>>>(ga, c->d_geo, d_chk);
+    std::vector<double> chk((size_t)Ne * 3);
+    cudaError_t err = cudaMemcpyAsync(chk.data(), d_chk, chk.size() * sizeof(double), cudaMemcpyDeviceToHost, c->st);
+    if (err == cudaSuccess) err = cudaStreamSynchronize(c->st);
+    cudaFree(d_chk);
+    if (err != cudaSuccess) { fail(CM_DG_ECUDA, std::string("metrics kernel: ") + cudaGetErrorString(err)); return bail(CM_DG_ECUDA); }
+    double minJ = 1e300, res = 0, mdx = 1e300;
+    for (int64_t e = 0; e < Ne; ++e) { minJ = std::min(minJ, chk[3 * e]); res = std::max(res, chk[3 * e + 1]); mdx = std::min(mdx, chk[3 * e + 2]); }
+    if (!(minJ > 0.0)) { fail(CM_DG_EINVAL, "cm_dg_setup: non-positive Jacobian determinant in the mesh"); return bail(CM_DG_EINVAL); }
+    if (res > 1e-10) {
+      char buf[160]; std::snprintf(buf, sizeof buf, "cm_dg_setup: discrete metric identity violated (%.3e > 1e-10): fully 3-D warps are not supported", res);
+      fail(CM_DG_EINVAL, buf); return bail(CM_DG_EINVAL);
+    }
+    c->min_node_dx = mdx;
+    kp.geo = c->d_geo;
+    if (p->use_ref) {
+      std::vector<double> tmp((size_t)3 * c->stride, 0.0);
+      const double* src[3] = {p->ref_rho, p->ref_rhoe, c->moist ? p->ref_rhoq : nullptr};
+      for (int a = 0; a < 3; ++a)
+        if (src[a])
+          for (int64_t e = 0; e < Ne; ++e)
+            std::memcpy(&tmp[(size_t)a * c->stride + (size_t)e * Np], src[a] + (size_t)c->lex_of_elem[e] * Np, Np * sizeof(double));
+      CM_CUDA_B(cudaMalloc(&c->d_ref, tmp.size() * sizeof(double)));
+      CM_CUDA_B(cudaMemcpy(c->d_ref, tmp.data(), tmp.size() * sizeof(double), cudaMemcpyHostToDevice));
+      kp.ref = c->d_ref;
+    }
+  }
+  (void)nn;
+
+  // ---- scratch owned by the ctx
+  if (p->sgs) CM_CUDA_B(cudaMalloc(&c->d_G, (size_t)c->ngrad * fbytes));
+  CM_CUDA_B(cudaMalloc(&c->d_part, (size_t)Ne * 7 * sizeof(double)));
+  // residual and ping-pong state are allocated on first use by cm_dg_lsrk_step
+
+  switch (Nq) {
+    case 3: c->launch_grad = cm_launch_gradient_nq3; c->launch_tend = cm_launch_tendency_nq3; break;
+    case 4: c->launch_grad = cm_launch_gradient_nq4; c->launch_tend = cm_launch_tendency_nq4; break;
+    case 5: c->launch_grad = cm_launch_gradient_nq5; c->launch_tend = cm_launch_tendency_nq5; break;
+    case 6: c->launch_grad = cm_launch_gradient_nq6; c->launch_tend = cm_launch_tendency_nq6; break;
+    case 7: c->launch_grad = cm_launch_gradient_nq7; c->launch_tend = cm_launch_tendency_nq7; break;
+    default: c->launch_grad = cm_launch_gradient_nq8; c->launch_tend = cm_launch_tendency_nq8; break;
+  }
+  CM_CUDA_B(cudaStreamSynchronize(c->st));
+  *out = c;
+  return CM_DG_OK;
+}
+
+int cm_dg_layout(const cm_dg_ctx* ctx, int64_t* n_elem, int32_t* np, int64_t* field_stride, int32_t* lex_of_elem) {
+  if (!ctx) return fail(CM_DG_EINVAL, "cm_dg_layout: NULL ctx");
+  if (n_elem) *n_elem = ctx->Ne;
+  if (np) *np = ctx->Np;
+  if (field_stride) *field_stride = ctx->stride;
+  if (lex_of_elem) std::memcpy(lex_of_elem, ctx->lex_of_elem.data(), (size_t)ctx->Ne * sizeof(int32_t));
+  return CM_DG_OK;
+}
+
+int cm_dg_coords(cm_dg_ctx* ctx, double* xyz_dev) {
+  if (!ctx || !xyz_dev) return fail(CM_DG_EINVAL, "cm_dg_coords: NULL argument");
+  GeoArgs ga = geo_args(ctx);
+  coords_kernel<<<(unsigned)ctx->Ne, 128, 0, ctx->st>>>(ga, xyz_dev);
+  CM_CUDA(cudaGetLastError());
+  return CM_DG_OK;
+}
+
+int cm_dg_metrics(cm_dg_ctx* ctx, double* Ja_dev, double* J_dev) {
+  if (!ctx || !Ja_dev || !J_dev) return fail(CM_DG_EINVAL, "cm_dg_metrics: NULL argument");
+  const long long n = ctx->Ne * ctx->Np;
+  const int thr = 256; const unsigned blocks = (unsigned)((n + thr - 1) / thr);
+  if (ctx->general)
+    general_metrics_copy<<<blocks, thr, 0, ctx->st>>>(n, ctx->stride, ctx->d_geo, Ja_dev, J_dev);
+  else
+    flat_metrics_fill<<<blocks, thr, 0, ctx->st>>>(n, ctx->stride, ctx->kp.cA[0], ctx->kp.cA[1], ctx->kp.cA[2], 1.0 / ctx->kp.invJ, Ja_dev, J_dev);
+  CM_CUDA(cudaGetLastError());
+  return CM_DG_OK;
+}
+
+int cm_dg_gradient(cm_dg_ctx* ctx, const double* Q_dev, double* G_dev) {
+  if (!ctx || !Q_dev || !G_dev) return fail(CM_DG_EINVAL, "cm_dg_gradient: NULL argument");
+  return run_gradient(ctx, Q_dev, G_dev, 1);
+}
+
+int cm_dg_rhs(cm_dg_ctx* ctx, const double* Q_dev, double* dQ_dev, double t) {
+  (void)t;   // no time-dependent forcing on this path (reading R14)
+  if (!ctx || !Q_dev || !dQ_dev) return fail(CM_DG_EINVAL, "cm_dg_rhs: NULL argument");
+  if (Q_dev == dQ_dev) return fail(CM_DG_EINVAL, "cm_dg_rhs: Q and dQ must be distinct buffers");
+  if (ctx->prm.sgs) { int rc = run_gradient(ctx, Q_dev, ctx->d_G, 0); if (rc) return rc; }
+  return run_tendency(ctx, Q_dev, dQ_dev, nullptr, 0, 0.0, 0.0, 0.0);
+}
+
+int cm_dg_lsrk_step(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t nsteps) {
+  (void)t;
+  if (!ctx || !Q_dev) return fail(CM_DG_EINVAL, "cm_dg_lsrk_step: NULL argument");
+  if (nsteps < 0) return fail(CM_DG_EINVAL, "cm_dg_lsrk_step: nsteps must be >= 0");
+  const size_t bytes = (size_t)ctx->nvar * ctx->stride * sizeof(double);
+  if (!ctx->d_res) CM_CUDA(cudaMalloc(&ctx->d_res, bytes));
+  if (!ctx->d_Q2) { CM_CUDA(cudaMalloc(&ctx->d_Q2, bytes)); CM_CUDA(cudaMemsetAsync(ctx->d_Q2, 0, bytes, ctx->st)); }
+  double* cur = Q_dev; double* oth = ctx->d_Q2;
+  for (int s = 0; s < nsteps; ++s)
+    for (int st = 0; st < 5; ++st) {
+      if (ctx->prm.sgs) { int rc = run_gradient(ctx, cur, ctx->d_G, 0); if (rc) return rc; }
+      int rc = run_tendency(ctx, cur, ctx->d_res, oth, 1, kRKA[st], kRKB[st], dt);
+      if (rc) return rc;
+      std::swap(cur, oth);
+    }
+  if (cur != Q_dev) {
+    Timed tm(ctx, 2);
+    CM_CUDA(cudaMemcpyAsync(Q_dev, cur, bytes, cudaMemcpyDeviceToDevice, ctx->st));
+  }
+  return CM_DG_OK;
+}
+
+int cm_dg_diagnostics(cm_dg_ctx* ctx, const double* Q_dev, cm_dg_diag* out) {
+  if (!ctx || !Q_dev || !out) return fail(CM_DG_EINVAL, "cm_dg_diagnostics: NULL argument");
+  DiagArgs a;
+  a.Nq = ctx->Nq; a.Np = ctx->Np; a.nvar = ctx->nvar; a.general = ctx->general; a.use_ref = ctx->prm.use_ref;
+  a.Ne = ctx->Ne; a.stride = ctx->stride; a.Q = Q_dev; a.geo = ctx->d_geo; a.erow = ctx->d_erow; a.ztab = ctx->d_ztab;
+  a.Jflat = 1.0 / ctx->kp.invJ; for (int i = 0; i < CM_MAXNQ; ++i) a.w[i] = ctx->w[i];
+  a.th = ctx->kp.th;
+  const int thr = 128;
+  {
+    Timed tm(ctx, 2);
+    diag_kernel<<<(unsigned)ctx->Ne, thr, 7 * thr * sizeof(double), ctx->st>>>(a, ctx->d_part);
+  }
+  CM_CUDA(cudaGetLastError());
+  std::vector<double> part((size_t)ctx->Ne * 7);
+  CM_CUDA(cudaMemcpyAsync(part.data(), ctx->d_part, part.size() * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
+  CM_CUDA(cudaStreamSynchronize(ctx->st));
+  double s[7] = {0, 0, 0, 0, 0, 0, 0};
+  for (int64_t e = 0; e < ctx->Ne; ++e)
+    for (int m = 0; m < 7; ++m) s[m] = (m == 5) ? std::max(s[m], part[7 * e + m]) : s[m] + part[7 * e + m];
+  out->mass = s[0]; out->energy = s[1]; out->water = s[2]; out->kinetic = s[3] / s[4]; out->volume = s[4];
+  out->max_wavespeed = s[5]; out->n_nonfinite = (int64_t)s[6]; out->min_node_dx = ctx->min_node_dx;
+  return CM_DG_OK;
+}
+
+static int stage_buffer(cm_dg_ctx* ctx, size_t bytes) {
+  if (!ctx->d_stage) CM_CUDA(cudaMalloc(&ctx->d_stage, 2 * bytes));
+  return CM_DG_OK;
+}
+
+int cm_dg_rhs_host(cm_dg_ctx* ctx, const double* Q_host, double* dQ_host, double t) {
+  if (!ctx || !Q_host || !dQ_host) return fail(CM_DG_EINVAL, "cm_dg_rhs_host: NULL argument");
+  const size_t bytes = (size_t)ctx->nvar * ctx->stride * sizeof(double);
+  int rc = stage_buffer(ctx, bytes); if (rc) return rc;
+  double* dq = ctx->d_stage; double* dd = ctx->d_stage + (size_t)ctx->nvar * ctx->stride;
+  CM_CUDA(cudaMemcpyAsync(dq, Q_host, bytes, cudaMemcpyHostToDevice, ctx->st));
+  rc = cm_dg_rhs(ctx, dq, dd, t); if (rc) return rc;
+  CM_CUDA(cudaMemcpyAsync(dQ_host, dd, bytes, cudaMemcpyDeviceToHost, ctx->st));
+  CM_CUDA(cudaStreamSynchronize(ctx->st));
+  return CM_DG_OK;
+}
+
+int cm_dg_lsrk_step_host(cm_dg_ctx* ctx, double* Q_host, double t, double dt, int32_t nsteps) {
+  if (!ctx || !Q_host) return fail(CM_DG_EINVAL, "cm_dg_lsrk_step_host: NULL argument");
+  const size_t bytes = (size_t)ctx->nvar * ctx->stride * sizeof(double);
+  int rc = stage_buffer(ctx, bytes); if (rc) return rc;
+  double* dq = ctx->d_stage;
+  CM_CUDA(cudaMemcpyAsync(dq, Q_host, bytes, cudaMemcpyHostToDevice, ctx->st));
+  rc = cm_dg_lsrk_step(ctx, dq, t, dt, nsteps); if (rc) return rc;
+  CM_CUDA(cudaMemcpyAsync(Q_host, dq, bytes, cudaMemcpyDeviceToHost, ctx->st));
+  CM_CUDA(cudaStreamSynchronize(ctx->st));
+  return CM_DG_OK;
+}
+
+int cm_dg_profile_begin(cm_dg_ctx* ctx) {
+  if (!ctx) return fail(CM_DG_EINVAL, "cm_dg_profile_begin: NULL ctx");
+  ctx->profiling = true; ctx->ev_used = 0;
+  return CM_DG_OK;
+}
+
+int cm_dg_profile_end(cm_dg_ctx* ctx, cm_dg_kernel_stats* out) {
+  if (!ctx || !out) return fail(CM_DG_EINVAL, "cm_dg_profile_end: NULL argument");
+  if (!ctx->profiling) return fail(CM_DG_ESTATE, "cm_dg_profile_end: profiling was not started");
+  ctx->profiling = false;
+  CM_CUDA(cudaStreamSynchronize(ctx->st));
+  std::memset(out, 0, sizeof(*out));
+  for (size_t k = 0; k + 1 < ctx->ev_used + 1 && k < ctx->ev_used; k += 2) {
+    float ms = 0.f;
+    CM_CUDA(cudaEventElapsedTime(&ms, ctx->ev[k], ctx->ev[k + 1]));
+    const int kind = ctx->ev_kind[k / 2];
+    if (kind == 0) { out->launches_gradient++; out->ms_gradient += ms; }
+    else if (kind == 1) { out->launches_tendency++; out->ms_tendency += ms; }
+    else { out->launches_other++; out->ms_other += ms; }
+  }
+  ctx->ev_used = 0;
+  return CM_DG_OK;
+}
+
+}  // extern "C"

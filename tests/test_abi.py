@@ -1,0 +1,69 @@
+"""CPU checks of the boundary: the C-ABI library builds for sm_100a, loads, exports every symbol that
+include/cm_dg.h declares, and fails loudly (no CPU fallback) when there is no CUDA device."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2110_00853_b200 import build
+    path = build.build()
+    return ctypes.CDLL(path)
+
+
+def test_header_symbols_are_exported(lib):
+    text = open(os.path.join(ROOT, "include", "cm_dg.h")).read()
+    names = set(re.findall(r"\b(cm_dg_[a-z_]+)\s*\(", text))
+    assert {"cm_dg_setup", "cm_dg_rhs", "cm_dg_lsrk_step", "cm_dg_diagnostics"} <= names
+    for n in names:
+        assert hasattr(lib, n), n
+    from paper_2110_00853_b200 import binding
+    assert set(binding.EXPORTS) == names
+
+
+def test_library_is_compiled_for_sm100a():
+    import subprocess
+    from paper_2110_00853_b200 import binding
+    out = subprocess.run(["cuobjdump", "--list-elf", binding.library_path()], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+
+
+def test_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("only meaningful on a machine without a GPU")
+    import paper_2110_00853_b200 as P
+    import workloads as W
+    cfg, Q, dt = W.config1()
+    with pytest.raises(P.CmDgError, match="no CUDA device"):
+        P.cm_dg_setup(cfg)
+
+
+def test_argument_validation_precedes_device_use():
+    import paper_2110_00853_b200 as P
+    import workloads as W
+    cfg, Q, dt = W.config1()
+    bad = dict(cfg); bad["N"] = 1
+    with pytest.raises(P.CmDgError, match="polynomial order"):
+        P.cm_dg_setup(bad)
+    bad = dict(cfg); bad["bc"] = (0, 2, 0)
+    with pytest.raises(P.CmDgError, match="bc"):
+        P.cm_dg_setup(bad)
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2110_00853_b200")
+    for dp, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                s = open(os.path.join(dp, f)).read()
+                assert "oracle" not in s.lower().replace("no cpu fallback", ""), os.path.join(dp, f)
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp")):
+            s = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2110_00853_b200" not in s and "cm_dg.h" not in s

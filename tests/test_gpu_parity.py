@@ -1,0 +1,170 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json's: 1e-11 per field for one RHS (reading R19), 1e-9 after
+100 LSRK54 steps.  Run on the B200 box with `pytest -m gpu`."""
+import numpy as np
+import pytest
+
+import workloads as W
+from parity_util import RHS_TOL, STEP_TOL, rhs_errors, small_config, state_errors
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2110_00853_b200 as pkg
+    return pkg
+
+
+def _pair(P, oracle_mod, cfg):
+    return oracle_mod.Oracle(cfg), P.CmDg(cfg)
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_coords_and_metrics(P, oracle_mod, k):
+    cfg, Q, dt = small_config(k)
+    o, g = _pair(P, oracle_mod, cfg)
+    x = g.to_host(g.coords())
+    xo = o.coords()
+    assert np.max(np.abs(x - xo)) <= 1e-13 * np.max(np.abs(xo))
+    Ja, J = g.metrics()
+    Ja = g.to_host(Ja); J = g.to_host(J)[..., 0]
+    for e in range(0, o.Ne, max(1, o.Ne // 17)):
+        go = o.elem_geometry(e)
+        sc = np.max(np.abs(go["Ja"]))
+        assert np.max(np.abs(Ja[e].reshape(-1, 3, 3) - go["Ja"])) <= 1e-12 * sc
+        assert np.max(np.abs(J[e] - go["J"])) <= 1e-12 * np.max(go["J"])
+
+
+@pytest.mark.parametrize("k", [2, 3, 4, 5])
+def test_gradient_parity(P, oracle_mod, k):
+    cfg, Q, dt = small_config(k)
+    if k == 4:
+        cfg["sgs"] = 1
+    o, g = _pair(P, oracle_mod, cfg)
+    Q = o.lsrk54(Q, dt, 3)            # a state with flow, so that every gradient is non-trivial
+    G = g.to_host(g.gradient(g.to_device(Q))).reshape(o.Ne, o.Np, 5, 3)
+    Go = o.gradient(Q)
+    for s in range(5 if cfg["nvar"] == 6 else 4):
+        scale = np.max(np.abs(Go[:, :, s]))
+        assert np.max(np.abs(G[:, :, s] - Go[:, :, s])) <= RHS_TOL * scale, s
+
+
+@pytest.mark.parametrize("N", [2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_rhs_parity(P, oracle_mod, k, N):
+    if N != 4 and k in (2, 3):
+        pytest.skip("other orders are covered on configs 1, 4, 5")
+    cfg, Q, dt = small_config(k, N=N)
+    o, g = _pair(P, oracle_mod, cfg)
+    dx = o.diagnostics(Q)["min_node_dx"]
+    for label, state in (("t0", Q), ("stepped", o.lsrk54(Q, dt, 5))):
+        dQ = g.to_host(g.rhs(g.to_device(state)))
+        dQo = o.rhs(state)
+        err = rhs_errors(dQ, dQo, cfg, state, dx)
+        assert np.all(err <= RHS_TOL), (label, err)
+
+
+def test_rhs_parity_general_path_on_flat_mesh(P, oracle_mod, monkeypatch):
+    """The stored-metric kernels must agree with the oracle on a flat mesh too (moist + SGS + walls)."""
+    monkeypatch.setenv("CM_DG_FORCE_GENERAL", "1")
+    cfg, Q, dt = small_config(5)
+    o, g = _pair(P, oracle_mod, cfg)
+    Q = o.lsrk54(Q, dt, 2)
+    err = rhs_errors(g.to_host(g.rhs(g.to_device(Q))), o.rhs(Q), cfg, Q, o.diagnostics(Q)["min_node_dx"])
+    assert np.all(err <= RHS_TOL), err
+
+
+def test_rhs_parity_lexicographic_order(P, oracle_mod, monkeypatch):
+    monkeypatch.setenv("CM_DG_ORDER", "lex")
+    cfg, Q, dt = small_config(3)
+    o, g = _pair(P, oracle_mod, cfg)
+    assert np.all(g.lex_of_elem == np.arange(o.Ne))
+    err = rhs_errors(g.to_host(g.rhs(g.to_device(Q))), o.rhs(Q), cfg, Q, o.diagnostics(Q)["min_node_dx"])
+    assert np.all(err <= RHS_TOL), err
+
+
+@pytest.mark.parametrize("k,nsteps", [(1, 10), (1, 100), (2, 100), (3, 100), (4, 100), (5, 100)])
+def test_lsrk_parity(P, oracle_mod, k, nsteps):
+    cfg, Q, dt = small_config(k)
+    o, g = _pair(P, oracle_mod, cfg)
+    Qd = g.to_device(Q)
+    g.lsrk_step(Qd, dt, nsteps)
+    Qo = o.lsrk54(Q, dt, nsteps)
+    err = state_errors(g.to_host(Qd), Qo)
+    assert np.all(err <= STEP_TOL), err
+    assert np.max(np.abs(Qo - Q)) > 0
+    # one RHS on the evolved state: every field now has a non-trivial tendency (R19)
+    e2 = rhs_errors(g.to_host(g.rhs(g.to_device(Qo))), o.rhs(Qo), cfg, Qo, o.diagnostics(Qo)["min_node_dx"])
+    assert np.all(e2 <= RHS_TOL), e2
+
+
+def test_lsrk_odd_and_even_step_counts_agree(P, oracle_mod):
+    """5*nsteps odd ends in the internal buffer and is copied back; both paths must give the same bits."""
+    cfg, Q, dt = small_config(1)
+    g = P.CmDg(cfg)
+    A = g.to_device(Q); B = g.to_device(Q)
+    g.lsrk_step(A, dt, 3)
+    g.lsrk_step(B, dt, 1); g.lsrk_step(B, dt, 2)
+    assert bool((A == B).all())
+
+
+@pytest.mark.parametrize("k", [2, 4, 5])
+def test_diagnostics_parity(P, oracle_mod, k):
+    cfg, Q, dt = small_config(k)
+    o, g = _pair(P, oracle_mod, cfg)
+    d = g.diagnostics(g.to_device(Q)); do = o.diagnostics(Q)
+    for key in ("mass", "energy", "water", "kinetic", "max_wavespeed", "min_node_dx", "volume"):
+        assert abs(d[key] - do[key]) <= 1e-12 * max(abs(do[key]), 1e-300), key
+    assert d["n_nonfinite"] == 0
+    Q2 = Q.copy(); Q2[3, 5, 1] = np.inf
+    assert g.diagnostics(g.to_device(Q2))["n_nonfinite"] == 1
+
+
+def test_host_entry_points(P, oracle_mod):
+    import torch
+    cfg, Q, dt = small_config(5)
+    g = P.CmDg(cfg)
+    Qh = torch.from_numpy(g.pack(Q)).pin_memory()
+    dQh = torch.zeros_like(Qh).pin_memory()
+    g.rhs_host(Qh, dQh)
+    assert bool((dQh.cuda() == g.rhs(g.to_device(Q))).all())
+    Qd = g.to_device(Q); g.lsrk_step(Qd, dt, 2)
+    g.lsrk_step_host(Qh, dt, 2)
+    assert bool((Qh.cuda() == Qd).all())
+
+
+def test_invariants_on_gpu(P, oracle_mod):
+    """Free stream on the warped mesh and steadiness of the reference state, checked on the CUDA path itself."""
+    cfg, Q, dt = small_config(4)
+    g = P.CmDg(cfg)
+    Qr = np.zeros_like(Q); Qr[..., 0] = cfg["ref_rho"]; Qr[..., 4] = cfg["ref_rhoe"]
+    dQ = g.to_host(g.rhs(g.to_device(Qr)))
+    assert np.max(np.abs(dQ[..., 1:4])) <= 1e-13 * 1.3 * 9.81
+    assert np.max(np.abs(dQ[..., 0])) == 0.0
+    cfg2 = dict(cfg); cfg2.update(grav=0.0, use_ref=0, bc=(0, 0, 0), sgs=1)
+    g2 = P.CmDg(cfg2)
+    z = W.node_coords(cfg2)[..., 2]; one = np.ones_like(z)
+    Qu = W.conserved(cfg2, 1.1 * one, 12.0 * one, -7.0 * one, 3.0 * one, 288.0 * one, 0 * one, z)
+    dQ = g2.to_host(g2.rhs(g2.to_device(Qu)))
+    dx = g2.diagnostics(g2.to_device(Qu))["min_node_dx"]
+    Tf = np.array([13.2, 1.1 * 144 + 1e5, 1.1 * 144 + 1e5, 1.1 * 144 + 1e5, 3.6e5 * 12]) / dx
+    for v in range(5):
+        assert np.max(np.abs(dQ[..., v])) <= 1e-13 * Tf[v], v
+
+
+def test_error_reporting(P):
+    cfg, Q, dt = small_config(1)
+    bad = dict(cfg); bad["N"] = 9
+    with pytest.raises(P.CmDgError):
+        P.CmDg(bad)
+    bad = dict(cfg); bad["nvar"] = 4
+    with pytest.raises(P.CmDgError):
+        P.CmDg(bad)
+    # inverted mesh: non-positive Jacobian must be rejected, not computed with
+    cfg4, _, _ = small_config(4)
+    bad = dict(cfg4); bad["zsfc_nodes"] = np.full_like(np.asarray(cfg4["zsfc_nodes"]), 5.0e4)
+    with pytest.raises(P.CmDgError):
+        P.CmDg(bad)
