@@ -48,7 +48,8 @@ def test_gradient_parity(P, oracle_mod, k):
     G = g.to_host(g.gradient(g.to_device(Q))).reshape(o.Ne, o.Np, 5, 3)
     Go = o.gradient(Q)
     for s in range(5 if cfg["nvar"] == 6 else 4):
-        scale = np.max(np.abs(Go[:, :, s]))
+        # one scale for the velocity-gradient tensor (v is identically ~0 in the slab configs)
+        scale = np.max(np.abs(Go[:, :, 0:3])) if s < 3 else np.max(np.abs(Go[:, :, s]))
         assert np.max(np.abs(G[:, :, s] - Go[:, :, s])) <= RHS_TOL * scale, s
 
 
