@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the fp64 DG right-hand side fused into LSRK54 on one B200 (BASELINE.json metric).
+
+A "step" is one LSRK54 time step of the whole hot path = 5 stages, each = auxiliary-gradient kernel +
+fused tendency/low-storage-update kernel (rows a1-a5 of the scope table), on BASELINE config 5:
+96x96x48 hexahedra at N=4, 6 prognostics, ~55.3 M nodes, moist Smagorinsky-Lilly, synthetic seeded state.
+value = nodes * 5 * K / time  [DOF-stages/s], whole job (all ranks).  The state (2.65 GB/copy) is far larger
+than the 126 MB L2, so no explicit L2 flush is needed between iterations.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--ne EX EY EZ] [--order N]
+
+N > 1 (torchrun): the path does not shard in this build ("replicas only"): each rank runs an independent
+replica on its own GPU, the timed region is bracketed by barriers and the max over ranks is taken.
+--impl reference: the CPU oracle (oracle/), as it stands, on the host cores of rank 0, on a bounded cut of
+the same workload (this tier's reference arm).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 DG RHS throughput (DOF-stages/s) at N=4; % of B200 HBM roofline"
+UNIT = "DOF-stages/s"
+# algorithmic bytes per node: each array once per sweep, fp64
+B_GRAD = {5: (5 + 9) * 8, 6: (6 + 12) * 8}                  # sweep A: read Q, write packed SGS fluxes
+B_TEND = {5: (5 + 9 + 5 + 5 + 5) * 8, 6: (6 + 12 + 6 + 6 + 6) * 8}   # sweep B: read Q, G, dQ; write dQ, Q
+B_TEND_STAGE1 = {5: (5 + 9 + 5 + 5) * 8, 6: (6 + 12 + 6 + 6) * 8}    # stage 1 (A_1 = 0) does not read dQ
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic():
+    """dram bytes per launch of the dominant kernel from the committed ncu capture, if one is recorded."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f).get("tendency_dram_bytes_per_launch")
+    return None
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index; self.rows = []; self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True); self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        pw = [float(r[2]) for r in self.rows if len(r) > 2 and r[2].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 3 + i and r[3 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
+
+
+def cut_of_config5(ne, order):
+    """Config 5 with the full 3 km column and the same element size, on an Ex x Ey x Ez brick."""
+    import workloads as W
+    full = W.SWEEP5[order]
+    hi = (6000.0 * ne[0] / full[0], 6000.0 * ne[1] / full[1], 3000.0 * ne[2] / full[2])
+    return W.config5(ne=tuple(ne), N=order, hi=hi)
+
+
+def time_oracle(sample_ne, order, steps, warmup=0):
+    """Times the CPU oracle (kind "oracle") on a cut of config 5; returns (DOF-stages/s, threads, description, s/step)."""
+    from oracle import oracle as om
+    cfg, Q, dt = cut_of_config5(sample_ne, order)
+    o = om.Oracle(cfg)
+    nodes = Q.shape[0] * Q.shape[1]
+    Qc = Q.copy(); dU = np.zeros_like(Q)
+    for _ in range(warmup):
+        for s in range(5):
+            o.lsrk54_stage(Qc, dU, dt, s)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        for s in range(5):
+            o.lsrk54_stage(Qc, dU, dt, s)
+    el = time.perf_counter() - t0
+    desc = "config 5 cut %dx%dx%d elements at N=%d (%d nodes, full 3 km column), %d LSRK54 steps" % (*sample_ne, order, nodes, steps)
+    return nodes * 5 * steps / el, om.num_threads(), desc, el / steps
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import workloads as W
+    full = W.SWEEP5[args.order]
+    sample = (full[0] // 4, full[1] // 4, full[2])          # 1/16 of the columns, full 3 km height
+    val, threads, desc, s_per_step = time_oracle(sample, args.order, args.steps, args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * s_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(args, sample_note="each step = one LSRK54 step on the bounded sample: " + desc),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def workload_config(args, sample_note=None):
+    ne = args.ne
+    c = {"workload": "BASELINE config 5: moist shallow-cumulus-shaped box, %dx%dx%d hexahedra, N=%d, 6 fp64 prognostics, "
+                     "Smagorinsky-Lilly, periodic x/y, no-flux z" % (ne[0], ne[1], ne[2], args.order),
+         "elements": int(np.prod(ne)), "nodes": int(np.prod(ne)) * (args.order + 1) ** 3, "order": args.order, "nvar": 6,
+         "step": "one LSRK54 step = 5 x (gradient kernel + fused tendency/update kernel)",
+         "l2": "inputs larger than L2 (state 2.65 GB per copy vs 126 MB L2), no flush needed",
+         "parallelism": "replicas only (one independent replica per GPU)"}
+    if sample_note:
+        c["sample"] = sample_note
+    return c
+
+
+def run_ours(args):
+    import torch
+    import workloads as W
+    import paper_2110_00853_b200 as P
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    t_gen = time.perf_counter()
+    cfg, Q, dt = cut_of_config5(args.ne, args.order)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        g = P.CmDg(cfg, stream=stream)
+        Qh = torch.from_numpy(g.pack(Q)).pin_memory()
+        del Q
+        Qd = Qh.to(g.device, non_blocking=True)
+    stream.synchronize()
+    t_gen = time.perf_counter() - t_gen
+    nodes = g.n_elem * g.np
+    nv = g.nvar
+    K, Wm = args.steps, args.warmup
+
+    # ---- device-resident throughput: K LSRK54 steps, CUDA events on the library stream
+    d0 = g.diagnostics(Qd)
+    for _ in range(Wm):
+        g.lsrk_step(Qd, dt, 1)
+    stream.synchronize()
+    sampler = ClockSampler(local); sampler.start()
+    time.sleep(0.3)
+    ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+    barrier()
+    g.profile_begin()
+    ev0.record(stream)
+    for _ in range(K):
+        g.lsrk_step(Qd, dt, 1)
+    ev1.record(stream)
+    stream.synchronize()
+    barrier()
+    ks = g.profile_end()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1)
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device=g.device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX); ms = float(t.item())
+    value = world * nodes * 5 * K / (ms * 1e-3)
+    d1 = g.diagnostics(Qd)
+
+    # ---- RHS alone (cm_dg_rhs), same state
+    dQ = g.empty(nv)
+    for _ in range(3):
+        g.rhs(Qd, dQ)
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    stream.synchronize(); e0.record(stream)
+    nrhs = max(5, K)
+    for _ in range(nrhs):
+        g.rhs(Qd, dQ)
+    e1.record(stream); stream.synchronize()
+    rhs_ms = e0.elapsed_time(e1) / nrhs
+    del dQ
+
+    # ---- end to end through the host-buffer C-ABI call: H2D + step + D2H inside the timed region
+    Ke = max(1, min(K, args.e2e_steps))
+    g.lsrk_step_host(Qh, dt, 1)                      # warm-up (allocates the staging buffer)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        g.lsrk_step_host(Qh, dt, 1)                  # synchronises the stream itself
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=g.device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX); e2e_s = float(t.item())
+    e2e_val = world * nodes * 5 * Ke / e2e_s
+    state_bytes = nv * g.stride * 8
+
+    # ---- roofline of the dominant kernel (fused tendency + LSRK update), measured live with CUDA events
+    peak, peak_src = measured_peaks()
+    n_t = max(1, ks["launches_tendency"]); n_g = max(1, ks["launches_gradient"])
+    t_tend = ks["ms_tendency"] / n_t; t_grad = ks["ms_gradient"] / n_g
+    bytes_tend = nodes * (4 * B_TEND[nv] + B_TEND_STAGE1[nv]) / 5.0
+    ach = bytes_tend / (t_tend * 1e-3) / 1e9
+    stage_bytes = nodes * (B_GRAD[nv] + (4 * B_TEND[nv] + B_TEND_STAGE1[nv]) / 5.0)
+    stage_gbs = stage_bytes * 5 * K / (ms * 1e-3) / 1e9
+    roof = {"bound": "hbm", "kernel": "cm_tendency_kernel (fused tendency + LSRK update)", "achieved": ach, "peak": peak,
+            "unit": "GB/s", "frac": ach / peak, "traffic": ncu_traffic(), "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": bytes_tend, "ms_per_launch": t_tend,
+            "share_of_step": ks["ms_tendency"] / (ks["ms_tendency"] + ks["ms_gradient"] + ks["ms_other"]),
+            "gradient_kernel": {"achieved": nodes * B_GRAD[nv] / (t_grad * 1e-3) / 1e9, "ms_per_launch": t_grad,
+                                "algorithmic_bytes_per_launch": nodes * B_GRAD[nv]},
+            "whole_stage": {"achieved": stage_gbs, "frac": stage_gbs / peak, "frac_of_8TBs_nominal": stage_gbs / 8000.0,
+                            "algorithmic_bytes_per_node_stage": stage_bytes / nodes},
+            "rhs_only": {"ms": rhs_ms, "dof_per_s": nodes / (rhs_ms * 1e-3),
+                         "achieved": nodes * (B_GRAD[nv] + B_TEND[nv] - nv * 16) / (rhs_ms * 1e-3) / 1e9}}
+    roof["rhs_only"]["frac"] = roof["rhs_only"]["achieved"] / peak
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": workload_config(args),
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes,
+                    "steps": Ke, "call": "cm_dg_lsrk_step_host (pinned host buffer)"},
+            "gpu_launches": int(ks["launches_gradient"] + ks["launches_tendency"] + ks["launches_other"]),
+            "clocks": clocks, "roofline": roof,
+            "conservation": {"rel_mass_change": (d1["mass"] - d0["mass"]) / d0["mass"],
+                             "rel_energy_change": (d1["energy"] - d0["energy"]) / d0["energy"],
+                             "n_nonfinite": d1["n_nonfinite"]},
+            "setup_s": t_gen}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        full = W.SWEEP5[args.order]
+        sample = (full[0] // 4, full[1] // 4, full[2]) if tuple(args.ne) == tuple(full) else tuple(args.ne)
+        val, threads, desc, _ = time_oracle(sample, args.order, 3)
+        line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--order", type=int, default=4, help="polynomial order N (config-5 sweep: 3..6)")
+    ap.add_argument("--ne", type=int, nargs=3, default=None, help="element counts (default: the full config-5 mesh)")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    import workloads as W
+    if args.ne is None:
+        args.ne = list(W.SWEEP5[args.order])
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
