@@ -15,6 +15,7 @@ struct CmThermo {
   double b;    // c_vv - c_vd
   double T_0, I_v0, grav;
   double dk;   // a c_vd - R_d b   (numerator of kappa - kappa_r, reading R12)
+  double icvd, kappa_d;  // 1 / c_vd, R_d / c_vd (dry air)
 };
 
 // Kernel argument block (passed by value, lives in the constant bank).
@@ -51,10 +52,11 @@ struct CmKP {
 struct CmLaunchCfg { int epb; int threads; size_t smem_grad; size_t smem_tend; };
 
 // implemented in cm_dg_kernels_inst.cu (one object per polynomial order)
-typedef cudaError_t (*cm_launch_fn)(const CmKP& kp, int moist, int general, cudaStream_t st);
+// variant: 1 = column-per-thread kernels (cm_dg_kernels.cuh), 2 = thread-per-node kernels (cm_dg_kernels2.cuh)
+typedef cudaError_t (*cm_launch_fn)(const CmKP& kp, int moist, int general, int variant, cudaStream_t st);
 #define CM_DECL_LAUNCHERS(NQ)                                                                 \
-  cudaError_t cm_launch_gradient_nq##NQ(const CmKP& kp, int moist, int general, cudaStream_t st); \
-  cudaError_t cm_launch_tendency_nq##NQ(const CmKP& kp, int moist, int general, cudaStream_t st);
+  cudaError_t cm_launch_gradient_nq##NQ(const CmKP& kp, int moist, int general, int variant, cudaStream_t st); \
+  cudaError_t cm_launch_tendency_nq##NQ(const CmKP& kp, int moist, int general, int variant, cudaStream_t st);
 CM_DECL_LAUNCHERS(3)
 CM_DECL_LAUNCHERS(4)
 CM_DECL_LAUNCHERS(5)

@@ -257,6 +257,7 @@ inline uint64_t spread3(uint64_t v) {
 struct cm_dg_ctx {
   cm_dg_params prm;
   int N, Nq, Np, nvar, ngrad, general, moist;
+  int variant = 2;   // kernel decomposition (env CM_DG_KERNEL=1 selects the column-per-thread kernels)
   int64_t Ne, stride;
   cudaStream_t st;
   std::vector<int32_t> lex_of_elem;
@@ -319,7 +320,7 @@ int run_gradient(cm_dg_ctx* c, const double* Q, double* Gout, int raw) {
   CmKP kp = c->kp;
   kp.Q = Q; kp.Gout = Gout; kp.mode = raw;
   Timed t(c, 0);
-  cudaError_t err = c->launch_grad(kp, c->moist, c->general, c->st);
+  cudaError_t err = c->launch_grad(kp, c->moist, c->general, c->variant, c->st);
   if (err != cudaSuccess) return fail(CM_DG_ECUDA, std::string("gradient kernel launch: ") + cudaGetErrorString(err));
   return CM_DG_OK;
 }
@@ -328,7 +329,7 @@ int run_tendency(cm_dg_ctx* c, const double* Q, double* dQ, double* Qnew, int mo
   CmKP kp = c->kp;
   kp.Q = Q; kp.G = c->d_G; kp.dQ = dQ; kp.Qnew = Qnew; kp.mode = mode; kp.rka = rka; kp.rkb = rkb; kp.dt = dt;
   Timed t(c, 1);
-  cudaError_t err = c->launch_tend(kp, c->moist, c->general, c->st);
+  cudaError_t err = c->launch_tend(kp, c->moist, c->general, c->variant, c->st);
   if (err != cudaSuccess) return fail(CM_DG_ECUDA, std::string("tendency kernel launch: ") + cudaGetErrorString(err));
   return CM_DG_OK;
 }
@@ -438,6 +439,7 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   }
   c->general = (p->geom != 0 || (p->use_ref && !ref_z_only)) ? 1 : 0;
   if (const char* fg = std::getenv("CM_DG_FORCE_GENERAL")) if (fg[0] == '1') c->general = 1;
+  if (const char* kv = std::getenv("CM_DG_KERNEL")) if (kv[0] == '1') c->variant = 1;
 
   auto bail = [&](int code) { free_ctx(c); return code; };
 #define CM_CUDA_B(call)                                                                                   \
@@ -477,6 +479,7 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   kp.th.R_d = p->R_d; kp.th.c_vd = p->c_vd; kp.th.a = p->R_v - p->R_d; kp.th.b = p->c_vv - p->c_vd;
   kp.th.T_0 = p->T_0; kp.th.I_v0 = p->I_v0; kp.th.grav = p->grav;
   kp.th.dk = kp.th.a * p->c_vd - p->R_d * kp.th.b;
+  kp.th.icvd = 1.0 / p->c_vd; kp.th.kappa_d = p->R_d / p->c_vd;
   kp.cA[0] = c->h[1] * c->h[2] / 4.0; kp.cA[1] = c->h[0] * c->h[2] / 4.0; kp.cA[2] = c->h[0] * c->h[1] / 4.0;
   kp.invJ = 8.0 / (c->h[0] * c->h[1] * c->h[2]);
   {
