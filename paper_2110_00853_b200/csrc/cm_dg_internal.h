@@ -6,6 +6,7 @@
 
 #define CM_MAXNQ 8
 #define CM_ZTAB_W 8   // doubles per z-table row (flat meshes): Phi, rho_r, rhoe_r, rhoq_r, E_r, q_r, 1/c_vm_r, unused
+#define CM_V3_MAXNQ 5 // largest Nq the TMA-ring kernels (cm_dg_kernels3.cuh) are built for (shared-memory footprint)
 #define CM_NGEO 12    // general geometry, per node: Ja[9], 1/J, z, (C_s Delta)^2
 
 // Thermodynamic constants of eq. (7)-(14) in the combinations the kernels use.
@@ -22,6 +23,8 @@ struct CmThermo {
 struct CmKP {
   // sizes
   int Ne;                // elements
+  int seg_len;           // v3 kernels: elements per x-segment (work unit), consecutive in library order
+  int n_units;           // v3 kernels: Ne / seg_len
   long long stride;      // field stride in doubles
   int sgs;               // Smagorinsky-Lilly on/off
   int use_ref;           // reference state removed (R12) or plain pressure
@@ -34,6 +37,7 @@ struct CmKP {
   double* Qnew;          // LSRK: updated state (ping-pong buffer)
   const int* nbr;        // [Ne][6] neighbour in library order, <0 = wall
   const int* erow;       // flat: [Ne] first z-table row of the element (= ez*Nq)
+  const int* elz;        // flat: [Ne][4] z-table rows {facing row of the -z neighbour, own first row, facing row of +z, 0}; -1 = wall
   const double* ztab;    // flat: [Ez*Nq][CM_ZTAB_W]
   const double* geo;     // general: [CM_NGEO][stride]
   const double* ref;     // general: [3][stride] rho_r, rhoe_r, rhoq_r
@@ -52,7 +56,8 @@ struct CmKP {
 struct CmLaunchCfg { int epb; int threads; size_t smem_grad; size_t smem_tend; };
 
 // implemented in cm_dg_kernels_inst.cu (one object per polynomial order)
-// variant: 1 = column-per-thread kernels (cm_dg_kernels.cuh), 2 = thread-per-node kernels (cm_dg_kernels2.cuh)
+// variant: 2 = thread-per-node kernels (cm_dg_kernels2.cuh; any geometry), 3 = persistent x-sweep kernels fed by
+// bulk TMA (cm_dg_kernels3.cuh; flat bricks, Nq <= 6)
 typedef cudaError_t (*cm_launch_fn)(const CmKP& kp, int moist, int general, int variant, cudaStream_t st);
 #define CM_DECL_LAUNCHERS(NQ)                                                                 \
   cudaError_t cm_launch_gradient_nq##NQ(const CmKP& kp, int moist, int general, int variant, cudaStream_t st); \

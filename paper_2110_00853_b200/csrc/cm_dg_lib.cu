@@ -243,28 +243,20 @@ __global__ void diag_kernel(const __grid_constant__ DiagArgs a, double* __restri
   }
 }
 
-// ------------------------------------------------------------------ element ordering
-// Library order: elements grouped in T x T x T tiles (x fastest inside a tile), tiles along a Morton curve,
-// so that the six face neighbours of an element are mostly a few KB..MB away (L2-resident traces).
-inline uint64_t spread3(uint64_t v) {
-  uint64_t r = 0;
-  for (int b = 0; b < 21; ++b) r |= ((v >> b) & 1ull) << (3 * b);
-  return r;
-}
-
 }  // namespace
 
 struct cm_dg_ctx {
   cm_dg_params prm;
   int N, Nq, Np, nvar, ngrad, general, moist;
-  int variant = 2;   // kernel decomposition (env CM_DG_KERNEL=1 selects the column-per-thread kernels)
+  int variant = 3;   // 3: TMA-ring x-sweep kernels (flat bricks, Nq <= 6); 2: thread-per-node kernels (env CM_DG_KERNEL=2)
+  int seg_len = 1;
   int64_t Ne, stride;
   cudaStream_t st;
   std::vector<int32_t> lex_of_elem;
   double xi[CM_MAXNQ], w[CM_MAXNQ], D[CM_MAXNQ][CM_MAXNQ];
   double h[3], min_node_dx;
   // device
-  int *d_nbr = nullptr, *d_erow = nullptr, *d_lex = nullptr;
+  int *d_nbr = nullptr, *d_erow = nullptr, *d_elz = nullptr, *d_lex = nullptr;
   double *d_ztab = nullptr, *d_geo = nullptr, *d_ref = nullptr, *d_G = nullptr, *d_res = nullptr, *d_Q2 = nullptr;
   double *d_zsfc = nullptr, *d_xyz_user = nullptr, *d_part = nullptr, *d_stage = nullptr;
   CmKP kp;
@@ -280,7 +272,7 @@ namespace {
 
 void free_ctx(cm_dg_ctx* c) {
   if (!c) return;
-  cudaFree(c->d_nbr); cudaFree(c->d_erow); cudaFree(c->d_lex); cudaFree(c->d_ztab); cudaFree(c->d_geo);
+  cudaFree(c->d_nbr); cudaFree(c->d_erow); cudaFree(c->d_elz); cudaFree(c->d_lex); cudaFree(c->d_ztab); cudaFree(c->d_geo);
   cudaFree(c->d_ref); cudaFree(c->d_G); cudaFree(c->d_res); cudaFree(c->d_Q2); cudaFree(c->d_zsfc);
   cudaFree(c->d_xyz_user); cudaFree(c->d_part); cudaFree(c->d_stage);
   for (auto e : c->ev) cudaEventDestroy(e);
@@ -316,7 +308,10 @@ struct Timed {
   }
 };
 
+bool misaligned(const void* ptr) { return (reinterpret_cast<uintptr_t>(ptr) & 15u) != 0; }
+
 int run_gradient(cm_dg_ctx* c, const double* Q, double* Gout, int raw) {
+  if (misaligned(Q) || misaligned(Gout)) return fail(CM_DG_EINVAL, "state arrays must be 16-byte aligned (bulk TMA source)");
   CmKP kp = c->kp;
   kp.Q = Q; kp.Gout = Gout; kp.mode = raw;
   Timed t(c, 0);
@@ -326,6 +321,7 @@ int run_gradient(cm_dg_ctx* c, const double* Q, double* Gout, int raw) {
 }
 
 int run_tendency(cm_dg_ctx* c, const double* Q, double* dQ, double* Qnew, int mode, double rka, double rkb, double dt) {
+  if (misaligned(Q) || misaligned(dQ) || misaligned(Qnew)) return fail(CM_DG_EINVAL, "state arrays must be 16-byte aligned (bulk TMA source)");
   CmKP kp = c->kp;
   kp.Q = Q; kp.G = c->d_G; kp.dQ = dQ; kp.Qnew = Qnew; kp.mode = mode; kp.rka = rka; kp.rkb = rkb; kp.dt = dt;
   Timed t(c, 1);
@@ -373,27 +369,31 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   c->N = p->N; c->Nq = Nq; c->Np = Np; c->nvar = p->nvar; c->moist = (p->nvar == 6);
   c->ngrad = c->moist ? 12 : 9;
   c->Ne = Ne;
-  c->stride = ((Ne * Np + 31) / 32) * 32;
+  c->stride = ((Ne * Np + 1 + 31) / 32) * 32;   // >= Ne*Np + 1: the bulk-TMA tile fetch of the last element reads one double past it
   c->st = (cudaStream_t)cuda_stream;
   for (int d = 0; d < 3; ++d) c->h[d] = (p->hi[d] - p->lo[d]) / p->ne[d];
   std::memset(c->D, 0, sizeof(c->D));
   lgl_operators(c->N, c->xi, c->w, c->D);
 
-  // ---- element order
+  // ---- element order (library order = schedule order of the x-sweep kernels)
+  // Work unit = segment of seg_len consecutive elements along x.  Units are ordered [y-patch][x-chunk][ez][ey in
+  // patch]: the one wave of persistent CTAs then works on a compact (y, z) patch of rows at the same x-chunk, so
+  // that y/z neighbour traces are in L2 when they are gathered (neighbours are 1 resp. PY units apart).
   {
     const char* ord = std::getenv("CM_DG_ORDER");
     const bool lex_order = ord && std::strcmp(ord, "lex") == 0;
-    const int T = 4;
+    int L = 1;
+    for (int d = 1; d <= p->ne[0] && d <= 32; ++d) if (p->ne[0] % d == 0) L = d;
+    if (L < 4 && p->ne[0] <= 128) L = p->ne[0];
+    if (const char* sl = std::getenv("CM_DG_SEGLEN")) { const int v = std::atoi(sl); if (v >= 1 && p->ne[0] % v == 0) L = v; }
+    int PY = 16;
+    if (const char* py = std::getenv("CM_DG_PATCH")) { const int v = std::atoi(py); if (v >= 1) PY = v; }
+    if (lex_order) { L = p->ne[0]; PY = p->ne[1]; }
+    c->seg_len = L;
     std::vector<std::pair<uint64_t, int32_t>> keys(Ne);
     for (int64_t l = 0; l < Ne; ++l) {
-      const int ex = (int)(l % p->ne[0]), ey = (int)((l / p->ne[0]) % p->ne[1]), ez = (int)(l / ((int64_t)p->ne[0] * p->ne[1]));
-      uint64_t key;
-      if (lex_order) key = (uint64_t)l;
-      else {
-        const uint64_t tile = spread3(ex / T) | (spread3(ey / T) << 1) | (spread3(ez / T) << 2);
-        const uint64_t local = (uint64_t)((ex % T) + T * ((ey % T) + T * (ez % T)));
-        key = (tile << 6) | local;
-      }
+      const uint64_t ex = (uint64_t)(l % p->ne[0]), ey = (uint64_t)((l / p->ne[0]) % p->ne[1]), ez = (uint64_t)(l / ((int64_t)p->ne[0] * p->ne[1]));
+      const uint64_t key = lex_order ? (uint64_t)l : (((((ey / PY) * (p->ne[0] / L) + ex / L) * p->ne[2] + ez) * PY + ey % PY) * L + ex % L);
       keys[l] = {key, (int32_t)l};
     }
     std::sort(keys.begin(), keys.end());
@@ -439,7 +439,8 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   }
   c->general = (p->geom != 0 || (p->use_ref && !ref_z_only)) ? 1 : 0;
   if (const char* fg = std::getenv("CM_DG_FORCE_GENERAL")) if (fg[0] == '1') c->general = 1;
-  if (const char* kv = std::getenv("CM_DG_KERNEL")) if (kv[0] == '1') c->variant = 1;
+  if (const char* kv = std::getenv("CM_DG_KERNEL")) if (kv[0] == '2') c->variant = 2;
+  if (c->general || Nq > CM_V3_MAXNQ) c->variant = 2;
 
   auto bail = [&](int code) { free_ctx(c); return code; };
 #define CM_CUDA_B(call)                                                                                   \
@@ -455,6 +456,17 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   CM_CUDA_B(cudaMalloc(&c->d_nbr, nbr.size() * sizeof(int32_t)));
   CM_CUDA_B(cudaMalloc(&c->d_erow, erow.size() * sizeof(int32_t)));
   CM_CUDA_B(cudaMalloc(&c->d_lex, (size_t)Ne * sizeof(int32_t)));
+  {
+    std::vector<int32_t> elz((size_t)Ne * 4, 0);
+    for (int64_t e = 0; e < Ne; ++e) {
+      const int32_t lo_nb = nbr[e * 6 + 4], hi_nb = nbr[e * 6 + 5];
+      elz[e * 4 + 0] = (lo_nb >= 0) ? erow[lo_nb] + Nq - 1 : -1;
+      elz[e * 4 + 1] = erow[e];
+      elz[e * 4 + 2] = (hi_nb >= 0) ? erow[hi_nb] : -1;
+    }
+    CM_CUDA_B(cudaMalloc(&c->d_elz, elz.size() * sizeof(int32_t)));
+    CM_CUDA_B(cudaMemcpy(c->d_elz, elz.data(), elz.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+  }
   CM_CUDA_B(cudaMemcpy(c->d_nbr, nbr.data(), nbr.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
   CM_CUDA_B(cudaMemcpy(c->d_erow, erow.data(), erow.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
   CM_CUDA_B(cudaMemcpy(c->d_lex, c->lex_of_elem.data(), (size_t)Ne * sizeof(int32_t), cudaMemcpyHostToDevice));
@@ -475,7 +487,7 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   // ---- kernel parameter block
   CmKP& kp = c->kp;
   std::memset(&kp, 0, sizeof(kp));
-  kp.Ne = (int)Ne; kp.stride = c->stride; kp.sgs = p->sgs ? 1 : 0; kp.use_ref = p->use_ref ? 1 : 0;
+  kp.Ne = (int)Ne; kp.seg_len = c->seg_len; kp.n_units = (int)(Ne / c->seg_len); kp.stride = c->stride; kp.sgs = p->sgs ? 1 : 0; kp.use_ref = p->use_ref ? 1 : 0;
   kp.th.R_d = p->R_d; kp.th.c_vd = p->c_vd; kp.th.a = p->R_v - p->R_d; kp.th.b = p->c_vv - p->c_vd;
   kp.th.T_0 = p->T_0; kp.th.I_v0 = p->I_v0; kp.th.grav = p->grav;
   kp.th.dk = kp.th.a * p->c_vd - p->R_d * kp.th.b;
@@ -490,7 +502,7 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   kp.shf = p->shf_bottom;
   kp.inv_w0 = 1.0 / c->w[0];
   for (int i = 0; i < CM_MAXNQ; ++i) for (int j = 0; j < CM_MAXNQ; ++j) kp.D[i][j] = c->D[i][j];
-  kp.nbr = c->d_nbr; kp.erow = c->d_erow;
+  kp.nbr = c->d_nbr; kp.erow = c->d_erow; kp.elz = c->d_elz;
 
   c->min_node_dx = std::min(c->h[0], std::min(c->h[1], c->h[2])) * 0.5 * (c->xi[1] - c->xi[0]);
 

@@ -78,6 +78,25 @@ def test_rhs_parity_general_path_on_flat_mesh(P, oracle_mod, monkeypatch):
     assert np.all(err <= RHS_TOL), err
 
 
+@pytest.mark.parametrize("env", [{"CM_DG_SEGLEN": "1"}, {"CM_DG_SEGLEN": "2", "CM_DG_PATCH": "2"}, {"CM_DG_SEGLEN": "3", "CM_DG_PATCH": "3"},
+                                 {"CM_DG_KERNEL": "2"}])
+@pytest.mark.parametrize("k", [1, 3, 5])
+def test_parity_schedule_variants(P, oracle_mod, monkeypatch, env, k):
+    """Segment length / patch width of the x-sweep kernels (segment ends take the global-trace path, interiors the
+    shared-memory path) and the thread-per-node kernels on flat meshes: RHS and 7 fused steps against the oracle."""
+    for key, val in env.items():
+        monkeypatch.setenv(key, val)
+    cfg, Q, dt = small_config(k)
+    o, g = _pair(P, oracle_mod, cfg)
+    Q1 = o.lsrk54(Q, dt, 2)
+    err = rhs_errors(g.to_host(g.rhs(g.to_device(Q1))), o.rhs(Q1), cfg, Q1, o.diagnostics(Q1)["min_node_dx"])
+    assert np.all(err <= RHS_TOL), err
+    Qd = g.to_device(Q)
+    g.lsrk_step(Qd, dt, 7)
+    err = state_errors(g.to_host(Qd), o.lsrk54(Q, dt, 7))
+    assert np.all(err <= STEP_TOL), err
+
+
 def test_rhs_parity_lexicographic_order(P, oracle_mod, monkeypatch):
     monkeypatch.setenv("CM_DG_ORDER", "lex")
     cfg, Q, dt = small_config(3)
