@@ -2,6 +2,8 @@
 // so that the orders build in parallel.  Exposes cm_launch_gradient_nq<NQ> / cm_launch_tendency_nq<NQ>.
 #include "cm_dg_kernels2.cuh"
 #include "cm_dg_kernels3.cuh"
+#include "cm_dg_kernels4.cuh"
+#include "cm_dg_kernels5.cuh"
 
 #ifndef CM_NQ
 #error "compile with -DCM_NQ=<N+1>"
@@ -10,6 +12,7 @@
 #define CM_CAT2(a, b) a##b
 #define CM_CAT(a, b) CM_CAT2(a, b)
 #define CM_HAS_V3 (CM_NQ <= CM_V3_MAXNQ)
+#define CM_HAS_V4 (CM_NQ <= CM_V4_MAXNQ)
 
 namespace {
 
@@ -103,9 +106,57 @@ cudaError_t launch_tend3(const CmKP& kp, cudaStream_t st) {
 }
 #endif
 
+template <int Nq, bool MOIST>
+cudaError_t launch_grad5(const CmKP& kp, cudaStream_t st) {
+  using C = CmCfg5<Nq, MOIST>;
+  static bool configured = false;
+  cudaError_t err = configure(cm5_gradient_kernel<Nq, MOIST>, C::GRAD_SMEM, configured);
+  if (err != cudaSuccess) return err;
+  cm5_gradient_kernel<Nq, MOIST><<<kp.Ne, C::THREADS, C::GRAD_SMEM, st>>>(kp);
+  return cudaGetLastError();
+}
+
+template <int Nq, bool MOIST, bool SGS>
+cudaError_t launch_tend5(const CmKP& kp, cudaStream_t st) {
+  using C = CmCfg5<Nq, MOIST>;
+  static bool configured = false;
+  cudaError_t err = configure(cm5_tendency_kernel<Nq, MOIST, SGS>, C::TEND_SMEM, configured);
+  if (err != cudaSuccess) return err;
+  cm5_tendency_kernel<Nq, MOIST, SGS><<<kp.Ne, C::THREADS, C::TEND_SMEM, st>>>(kp);
+  return cudaGetLastError();
+}
+
+#if CM_HAS_V4
+template <int Nq, bool MOIST>
+cudaError_t launch_grad4(const CmKP& kp, cudaStream_t st) {
+  using C = CmCfg4<Nq, MOIST>;
+  static bool configured = false;
+  cudaError_t err = configure(cm4_gradient_kernel<Nq, MOIST>, C::GRAD_SMEM, configured);
+  if (err != cudaSuccess) return err;
+  const int per_cta = C::WG * kp.epw;
+  cm4_gradient_kernel<Nq, MOIST><<<(kp.Ne + per_cta - 1) / per_cta, 32 * C::WG, C::GRAD_SMEM, st>>>(kp);
+  return cudaGetLastError();
+}
+
+template <int Nq, bool MOIST, bool SGS>
+cudaError_t launch_tend4(const CmKP& kp, cudaStream_t st) {
+  using C = CmCfg4<Nq, MOIST>;
+  static bool configured = false;
+  cudaError_t err = configure(cm4_tendency_kernel<Nq, MOIST, SGS>, C::TEND_SMEM, configured);
+  if (err != cudaSuccess) return err;
+  const int per_cta = C::WT * kp.epw;
+  cm4_tendency_kernel<Nq, MOIST, SGS><<<(kp.Ne + per_cta - 1) / per_cta, 32 * C::WT, C::TEND_SMEM, st>>>(kp);
+  return cudaGetLastError();
+}
+#endif
+
 }  // namespace
 
 cudaError_t CM_CAT(cm_launch_gradient_nq, CM_NQ)(const CmKP& kp, int moist, int general, int variant, cudaStream_t st) {
+  if (variant == 5 && !general) return moist ? launch_grad5<CM_NQ, true>(kp, st) : launch_grad5<CM_NQ, false>(kp, st);
+#if CM_HAS_V4
+  if (variant == 4 && !general) return moist ? launch_grad4<CM_NQ, true>(kp, st) : launch_grad4<CM_NQ, false>(kp, st);
+#endif
 #if CM_HAS_V3
   if (variant == 3 && !general) return moist ? launch_grad3<CM_NQ, true>(kp, st) : launch_grad3<CM_NQ, false>(kp, st);
 #endif
@@ -114,6 +165,16 @@ cudaError_t CM_CAT(cm_launch_gradient_nq, CM_NQ)(const CmKP& kp, int moist, int 
 }
 
 cudaError_t CM_CAT(cm_launch_tendency_nq, CM_NQ)(const CmKP& kp, int moist, int general, int variant, cudaStream_t st) {
+  if (variant == 5 && !general) {
+    if (kp.sgs) return moist ? launch_tend5<CM_NQ, true, true>(kp, st) : launch_tend5<CM_NQ, false, true>(kp, st);
+    return moist ? launch_tend5<CM_NQ, true, false>(kp, st) : launch_tend5<CM_NQ, false, false>(kp, st);
+  }
+#if CM_HAS_V4
+  if (variant == 4 && !general) {
+    if (kp.sgs) return moist ? launch_tend4<CM_NQ, true, true>(kp, st) : launch_tend4<CM_NQ, false, true>(kp, st);
+    return moist ? launch_tend4<CM_NQ, true, false>(kp, st) : launch_tend4<CM_NQ, false, false>(kp, st);
+  }
+#endif
 #if CM_HAS_V3
   if (variant == 3 && !general) {
     if (kp.sgs) return moist ? launch_tend3<CM_NQ, true, true>(kp, st) : launch_tend3<CM_NQ, false, true>(kp, st);

@@ -248,7 +248,8 @@ __global__ void diag_kernel(const __grid_constant__ DiagArgs a, double* __restri
 struct cm_dg_ctx {
   cm_dg_params prm;
   int N, Nq, Np, nvar, ngrad, general, moist;
-  int variant = 3;   // 3: TMA-ring x-sweep kernels (flat bricks, Nq <= 6); 2: thread-per-node kernels (env CM_DG_KERNEL=2)
+  int variant = 5;   // 4: warp-per-element kernels (flat bricks, Nq <= 6); 3: TMA-ring x-sweep kernels (flat, Nq <= 5); 2: thread-per-node
+                     // kernels (any geometry); env CM_DG_KERNEL=2|3|4 overrides
   int seg_len = 1;
   int64_t Ne, stride;
   cudaStream_t st;
@@ -439,8 +440,8 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   }
   c->general = (p->geom != 0 || (p->use_ref && !ref_z_only)) ? 1 : 0;
   if (const char* fg = std::getenv("CM_DG_FORCE_GENERAL")) if (fg[0] == '1') c->general = 1;
-  if (const char* kv = std::getenv("CM_DG_KERNEL")) if (kv[0] == '2') c->variant = 2;
-  if (c->general || Nq > CM_V3_MAXNQ) c->variant = 2;
+  if (const char* kv = std::getenv("CM_DG_KERNEL")) if (kv[0] >= '2' && kv[0] <= '5') c->variant = kv[0] - '0';
+  if (c->general || (c->variant == 3 && Nq > CM_V3_MAXNQ) || (c->variant == 4 && Nq > CM_V4_MAXNQ)) c->variant = 2;
 
   auto bail = [&](int code) { free_ctx(c); return code; };
 #define CM_CUDA_B(call)                                                                                   \
@@ -487,6 +488,8 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   // ---- kernel parameter block
   CmKP& kp = c->kp;
   std::memset(&kp, 0, sizeof(kp));
+  kp.epw = 4;
+  if (const char* ev = std::getenv("CM_DG_EPW")) { const int v = std::atoi(ev); if (v >= 1) kp.epw = v; }
   kp.Ne = (int)Ne; kp.seg_len = c->seg_len; kp.n_units = (int)(Ne / c->seg_len); kp.stride = c->stride; kp.sgs = p->sgs ? 1 : 0; kp.use_ref = p->use_ref ? 1 : 0;
   kp.th.R_d = p->R_d; kp.th.c_vd = p->c_vd; kp.th.a = p->R_v - p->R_d; kp.th.b = p->c_vv - p->c_vd;
   kp.th.T_0 = p->T_0; kp.th.I_v0 = p->I_v0; kp.th.grav = p->grav;
