@@ -6,8 +6,6 @@
 
 #define CM_MAXNQ 8
 #define CM_ZTAB_W 8   // doubles per z-table row (flat meshes): Phi, rho_r, rhoe_r, rhoq_r, E_r, q_r, 1/c_vm_r, unused
-#define CM_V4_MAXNQ 6 // largest Nq the warp-per-element kernels (cm_dg_kernels4.cuh) are used for
-#define CM_V3_MAXNQ 5 // largest Nq the TMA-ring kernels (cm_dg_kernels3.cuh) are built for (shared-memory footprint)
 #define CM_NGEO 12    // general geometry, per node: Ja[9], 1/J, z, (C_s Delta)^2
 
 // Thermodynamic constants of eq. (7)-(14) in the combinations the kernels use.
@@ -24,9 +22,10 @@ struct CmThermo {
 struct CmKP {
   // sizes
   int Ne;                // elements
-  int seg_len;           // v3 kernels: elements per x-segment (work unit), consecutive in library order
-  int n_units;           // v3 kernels: Ne / seg_len
-  int epw;               // v4 kernels: consecutive elements each warp walks through
+  // tiled element order e = ((((ey / gPY) * gNXC + ex / gL) * gEz + ez) * gPY + ey % gPY) * gL + ex % gL
+  int gL, gPY, gNXC, gNYP, gEz;   // x-chunk length (divides Ex), y-patch height (divides Ey), Ex / gL, Ey / gPY, Ez
+  int gbc[3];            // per direction: 1 = walls, 0 = periodic
+  float ginvL, ginvNXC;  // 1 / gL, 1 / gNXC (exact small-integer division in cm7_position)
   long long stride;      // field stride in doubles
   int sgs;               // Smagorinsky-Lilly on/off
   int use_ref;           // reference state removed (R12) or plain pressure
@@ -58,8 +57,8 @@ struct CmKP {
 struct CmLaunchCfg { int epb; int threads; size_t smem_grad; size_t smem_tend; };
 
 // implemented in cm_dg_kernels_inst.cu (one object per polynomial order)
-// variant: 2 = thread-per-node kernels (cm_dg_kernels2.cuh; any geometry), 3 = persistent x-sweep kernels fed by
-// bulk TMA (cm_dg_kernels3.cuh; flat bricks, Nq <= 5), 4 = warp-per-element kernels (cm_dg_kernels4.cuh; flat bricks)
+// variant: 2 = thread-per-node kernels (cm_dg_kernels2.cuh; any geometry), 7 = CTA-per-element kernels fed by bulk TMA
+// and cp.async (cm_dg_kernels7.cuh; flat bricks)
 typedef cudaError_t (*cm_launch_fn)(const CmKP& kp, int moist, int general, int variant, cudaStream_t st);
 #define CM_DECL_LAUNCHERS(NQ)                                                                 \
   cudaError_t cm_launch_gradient_nq##NQ(const CmKP& kp, int moist, int general, int variant, cudaStream_t st); \

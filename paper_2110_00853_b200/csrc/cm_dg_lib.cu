@@ -248,9 +248,8 @@ __global__ void diag_kernel(const __grid_constant__ DiagArgs a, double* __restri
 struct cm_dg_ctx {
   cm_dg_params prm;
   int N, Nq, Np, nvar, ngrad, general, moist;
-  int variant = 5;   // 4: warp-per-element kernels (flat bricks, Nq <= 6); 3: TMA-ring x-sweep kernels (flat, Nq <= 5); 2: thread-per-node
-                     // kernels (any geometry); env CM_DG_KERNEL=2|3|4 overrides
-  int seg_len = 1;
+  int variant = 7;   // 7: CTA-per-element kernels, all inputs staged asynchronously (cm_dg_kernels7.cuh; flat bricks);
+                     // 2: thread-per-node kernels (cm_dg_kernels2.cuh; any geometry); env CM_DG_KERNEL=2 forces the latter
   int64_t Ne, stride;
   cudaStream_t st;
   std::vector<int32_t> lex_of_elem;
@@ -376,30 +375,28 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   std::memset(c->D, 0, sizeof(c->D));
   lgl_operators(c->N, c->xi, c->w, c->D);
 
-  // ---- element order (library order = schedule order of the x-sweep kernels)
-  // Work unit = segment of seg_len consecutive elements along x.  Units are ordered [y-patch][x-chunk][ez][ey in
-  // patch]: the one wave of persistent CTAs then works on a compact (y, z) patch of rows at the same x-chunk, so
-  // that y/z neighbour traces are in L2 when they are gathered (neighbours are 1 resp. PY units apart).
+  // ---- element order (library order = launch order of the CTA-per-element kernels)
+  // e = ((((ey / PY) * NXC + ex / L) * Ez + ez) * PY + ey % PY) * L + ex % L with L | Ex, PY | Ey: consecutive CTAs
+  // walk up a column of (PY x L)-element tiles, so that the one wave of resident CTAs works on a compact brick and
+  // the x/y/z neighbour traces are in L2 when they are gathered (a z neighbour is PY*L elements away, a y/x
+  // neighbour at most Ez*PY*L).  The flat kernels recompute this map from blockIdx (cm6_position).
+  int L = 1, PY = 1;
   {
     const char* ord = std::getenv("CM_DG_ORDER");
     const bool lex_order = ord && std::strcmp(ord, "lex") == 0;
-    int L = 1;
-    for (int d = 1; d <= p->ne[0] && d <= 32; ++d) if (p->ne[0] % d == 0) L = d;
-    if (L < 4 && p->ne[0] <= 128) L = p->ne[0];
-    if (const char* sl = std::getenv("CM_DG_SEGLEN")) { const int v = std::atoi(sl); if (v >= 1 && p->ne[0] % v == 0) L = v; }
-    int PY = 16;
-    if (const char* py = std::getenv("CM_DG_PATCH")) { const int v = std::atoi(py); if (v >= 1) PY = v; }
+    int maxL = 32, maxPY = 16;
+    if (const char* sl = std::getenv("CM_DG_SEGLEN")) { const int v = std::atoi(sl); if (v >= 1) maxL = v; }
+    if (const char* py = std::getenv("CM_DG_PATCH")) { const int v = std::atoi(py); if (v >= 1) maxPY = v; }
+    for (int d = 1; d <= p->ne[0] && d <= maxL; ++d) if (p->ne[0] % d == 0) L = d;
+    for (int d = 1; d <= p->ne[1] && d <= maxPY; ++d) if (p->ne[1] % d == 0) PY = d;
     if (lex_order) { L = p->ne[0]; PY = p->ne[1]; }
-    c->seg_len = L;
-    std::vector<std::pair<uint64_t, int32_t>> keys(Ne);
-    for (int64_t l = 0; l < Ne; ++l) {
-      const uint64_t ex = (uint64_t)(l % p->ne[0]), ey = (uint64_t)((l / p->ne[0]) % p->ne[1]), ez = (uint64_t)(l / ((int64_t)p->ne[0] * p->ne[1]));
-      const uint64_t key = lex_order ? (uint64_t)l : (((((ey / PY) * (p->ne[0] / L) + ex / L) * p->ne[2] + ez) * PY + ey % PY) * L + ex % L);
-      keys[l] = {key, (int32_t)l};
-    }
-    std::sort(keys.begin(), keys.end());
     c->lex_of_elem.resize(Ne);
-    for (int64_t e = 0; e < Ne; ++e) c->lex_of_elem[e] = keys[e].second;
+    const int NXC = p->ne[0] / L;
+    for (int64_t l = 0; l < Ne; ++l) {
+      const int64_t ex = l % p->ne[0], ey = (l / p->ne[0]) % p->ne[1], ez = l / ((int64_t)p->ne[0] * p->ne[1]);
+      const int64_t e = ((((ey / PY) * NXC + ex / L) * p->ne[2] + ez) * PY + ey % PY) * L + ex % L;
+      c->lex_of_elem[e] = (int32_t)l;
+    }
   }
   std::vector<int32_t> pos_of_lex(Ne);
   for (int64_t e = 0; e < Ne; ++e) pos_of_lex[c->lex_of_elem[e]] = (int32_t)e;
@@ -440,8 +437,8 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   }
   c->general = (p->geom != 0 || (p->use_ref && !ref_z_only)) ? 1 : 0;
   if (const char* fg = std::getenv("CM_DG_FORCE_GENERAL")) if (fg[0] == '1') c->general = 1;
-  if (const char* kv = std::getenv("CM_DG_KERNEL")) if (kv[0] >= '2' && kv[0] <= '5') c->variant = kv[0] - '0';
-  if (c->general || (c->variant == 3 && Nq > CM_V3_MAXNQ) || (c->variant == 4 && Nq > CM_V4_MAXNQ)) c->variant = 2;
+  if (const char* kv = std::getenv("CM_DG_KERNEL")) if (kv[0] == '2' || kv[0] == '7') c->variant = kv[0] - '0';
+  if (c->general) c->variant = 2;
 
   auto bail = [&](int code) { free_ctx(c); return code; };
 #define CM_CUDA_B(call)                                                                                   \
@@ -488,9 +485,14 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   // ---- kernel parameter block
   CmKP& kp = c->kp;
   std::memset(&kp, 0, sizeof(kp));
-  kp.epw = 4;
-  if (const char* ev = std::getenv("CM_DG_EPW")) { const int v = std::atoi(ev); if (v >= 1) kp.epw = v; }
-  kp.Ne = (int)Ne; kp.seg_len = c->seg_len; kp.n_units = (int)(Ne / c->seg_len); kp.stride = c->stride; kp.sgs = p->sgs ? 1 : 0; kp.use_ref = p->use_ref ? 1 : 0;
+  kp.ginvL = 1.0f / (float)L; kp.ginvNXC = 1.0f / (float)(p->ne[0] / L);
+  kp.gL = L; kp.gPY = PY; kp.gNXC = p->ne[0] / L; kp.gNYP = p->ne[1] / PY; kp.gEz = p->ne[2];
+  for (int d = 0; d < 3; ++d) kp.gbc[d] = p->bc[d];
+  if ((int64_t)PY * L > 2147483647LL || p->ne[2] > 65535 || (int64_t)kp.gNXC * kp.gNYP > 65535) {
+    fail(CM_DG_EINVAL, "cm_dg_setup: mesh exceeds the launch-grid limits (Ez and (Ex/L)*(Ey/PY) must be <= 65535)");
+    return bail(CM_DG_EINVAL);
+  }
+  kp.Ne = (int)Ne; kp.stride = c->stride; kp.sgs = p->sgs ? 1 : 0; kp.use_ref = p->use_ref ? 1 : 0;
   kp.th.R_d = p->R_d; kp.th.c_vd = p->c_vd; kp.th.a = p->R_v - p->R_d; kp.th.b = p->c_vv - p->c_vd;
   kp.th.T_0 = p->T_0; kp.th.I_v0 = p->I_v0; kp.th.grav = p->grav;
   kp.th.dk = kp.th.a * p->c_vd - p->R_d * kp.th.b;
