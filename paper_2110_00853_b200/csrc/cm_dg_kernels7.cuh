@@ -71,9 +71,13 @@ template <int Nq, bool MOIST> struct CmCfg7 {
   static constexpr int NFP = ((NF + 31) / 32) * 32;         // line tasks of one direction, padded to whole warps
   static constexpr int ZR = Nq + 2;                         // z-table rows: facing row below, own Nq rows, facing row above
   static constexpr int TAIL = ZR * CM_ZTAB_W + 2;           // z rows, mbarrier
-  static constexpr int TEND_DOUBLES = (NV + 3 * NV + 1 + NV) * SLOT + 6 * NTR * NF + TAIL;   // Q, F^1..3 (G in F^1,F^2), c, residual, traces
-  static constexpr int GRAD_DOUBLES = (NV + 3 * NS) * SLOT + 6 * NV * NF + TAIL;             // Q (then s in place), ds/dxi_d, traces
-  static_assert(3 * NV >= NG, "the packed SGS fluxes are staged in the flux tiles");
+  // stride between the trace blocks of two faces: >= rows * NF and = NF (mod 16), so that consecutive face nodes of a
+  // warp that straddles two faces fall into consecutive banks
+  static constexpr int fstride(int rows) { return rows * NF + ((NF - rows * NF) % 16 + 16) % 16; }
+  static constexpr int TS_T = fstride(NTR), TS_G = fstride(NV);
+  static constexpr int TEND_DOUBLES = (NV + 3 * NV + 1 + NV) * SLOT + 6 * TS_T + TAIL;   // Q, F^1 F^3 F^2 (G lands in F^1,F^3), c, residual, traces
+  static constexpr int GRAD_DOUBLES = (NV + 3 * NS) * SLOT + 6 * TS_G + TAIL;            // Q (then s in place), ds/dxi_d, traces
+  static_assert(2 * NV >= NG, "the packed SGS fluxes are staged in the F^1, F^3 tiles");
   static constexpr size_t TEND_SMEM = sizeof(double) * TEND_DOUBLES;
   static constexpr size_t GRAD_SMEM = sizeof(double) * GRAD_DOUBLES;
   static constexpr int fit(size_t smem) { return (int)(233472 / (smem + 1024)); }
@@ -167,8 +171,8 @@ __device__ __forceinline__ void cm7_face_node(int fn, int& f, int& m, int& d, in
 }
 
 // CTA prologue shared by both kernels: z rows and neighbour traces to shared memory by cp.async.
-//   T[(f * NT + v) * NF + m]: value v of the node of neighbour f that coincides with face node m of face f
-template <int Nq, int NV, int NGD, int NT, int THREADS>
+//   T[f * TS + v * NF + m]: value v of the node of neighbour f that coincides with face node m of face f
+template <int Nq, int NV, int NGD, int TS, int THREADS>
 __device__ __forceinline__ void cm7_prefetch_traces(const CmKP& p, const Cm7Pos& q, int t, double* __restrict__ T,
                                                     double* __restrict__ zt) {
   constexpr int NF = Nq * Nq, NP = NF * Nq, ZR = Nq + 2;
@@ -188,7 +192,7 @@ __device__ __forceinline__ void cm7_prefetch_traces(const CmKP& p, const Cm7Pos&
     if (!((q.wallmask >> f) & 1)) {
       const int nb = cm7_neighbour(p, q, d, s);
       const size_t idp = (size_t)nb * NP + np_;
-      double* dst = T + f * (NT * NF) + m;
+      double* dst = T + f * TS + m;
       const double* src = p.Q + idp;
 #pragma unroll
       for (int v = 0; v < NV; ++v) { cm7_cp8(dst + v * NF, src); src += p.stride; }
@@ -212,12 +216,11 @@ template <int Nq, bool MOIST, bool SGS>
 __device__ __forceinline__ void cm7_tend_face(const CmKP& p, const double* __restrict__ Qs, const double* __restrict__ cs,
                                               double* __restrict__ T, const double* __restrict__ zt, int wallmask, int fn) {
   using C = CmCfg7<Nq, MOIST>;
-  constexpr int NF = C::NF, NV = C::NV, NGD = C::NGD, SLOT = C::SLOT;
-  constexpr int NT = SGS ? C::NTR : NV;
+  constexpr int NF = C::NF, NV = C::NV, NGD = C::NGD, SLOT = C::SLOT, TS = C::TS_T;
   int f, m, d, s, nm, np_, kline;
   cm7_face_node<Nq>(fn, f, m, d, s, nm, np_, kline);
   const bool wall = (wallmask >> f) & 1;
-  double* tr = T + f * (NT * NF) + m;
+  double* tr = T + f * TS + m;
   const double sgn = s ? 1.0 : -1.0;
   const double sJ = (d == 0) ? p.cA[0] : (d == 1) ? p.cA[1] : p.cA[2];
   const double A = sgn * sJ;
@@ -271,14 +274,14 @@ __device__ __forceinline__ void cm7_tend_face(const CmKP& p, const double* __res
   for (int v = 0; v < NV; ++v) tr[v * NF] = rf[v];
 }
 
-// tendency, phase 2b: line task.  Fd = the NV tiles holding F^D; on return the line holds D_D F^D minus the lifted
+// tendency, phase 2b: line task.  Fd = the NV tiles holding F^D (F^2 tiles are stored with i and j swapped, so the
+// eta-lines are contiguous like the xi-lines: no bank conflicts in any direction); on return the line holds D_D F^D minus the lifted
 // own-side half of the face term at its two ends (eq. 32)
 template <int Nq, bool MOIST, int D>
 __device__ __forceinline__ void cm7_tend_line(const CmKP& p, double* __restrict__ Fd, int wallmask, int l) {
   using C = CmCfg7<Nq, MOIST>;
-  constexpr int NF = C::NF, N = Nq - 1, NV = C::NV, SLOT = C::SLOT, STR = Cm7Str<Nq, D>::value;
-  const int b = l / Nq, a = l - b * Nq;
-  const int base = (D == 0) ? Nq * l : (D == 1) ? a + NF * b : l;
+  constexpr int N = Nq - 1, NV = C::NV, SLOT = C::SLOT, STR = (D == 2) ? Nq * Nq : 1;   // F^2 tiles: i, j swapped
+  const int base = (D == 2) ? l : Nq * l;
   const double c0 = p.inv_w0 * (((wallmask >> (2 * D)) & 1) ? 1.0 : 0.5);      // -sgn = +1 at the low end
   const double cN = -p.inv_w0 * (((wallmask >> (2 * D + 1)) & 1) ? 1.0 : 0.5);
 #pragma unroll
@@ -306,14 +309,14 @@ template <int Nq, bool MOIST, bool SGS, int MODE>
 __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>::MINB_T) cm7_tendency_kernel(const __grid_constant__ CmKP p) {
   using C = CmCfg7<Nq, MOIST>;
   constexpr int NF = C::NF, NP = C::NP, N = Nq - 1, NV = C::NV, NG = C::NG, SLOT = C::SLOT, NFP = C::NFP, THREADS = C::THREADS;
-  constexpr int NT = SGS ? C::NTR : NV;
+  constexpr int TS = C::TS_T;
   extern __shared__ __align__(128) double smem7[];
   double* Qt = smem7;                                  // [NV][SLOT]     state
-  double* Ft = Qt + NV * SLOT;                         // [3][NV][SLOT]  F^1, F^2, F^3 (the packed SGS fluxes G land in F^1, F^2)
+  double* Ft = Qt + NV * SLOT;                         // [3][NV][SLOT]  F^1, F^3 (the packed SGS fluxes G land here), F^2 (i, j swapped)
   double* ct = Ft + 3 * NV * SLOT;                     // [SLOT]         sound speed
   double* Rt = ct + SLOT;                              // [NV][SLOT]     LSRK residual
-  double* T = Rt + NV * SLOT;                          // [6][NTR][NF]   neighbour traces, then rf
-  double* zt = T + 6 * C::NTR * NF;                    // [ZR][CM_ZTAB_W]
+  double* T = Rt + NV * SLOT;                          // [6][TS]        neighbour traces [v][m] per face, then rf
+  double* zt = T + 6 * TS;                    // [ZR][CM_ZTAB_W]
   uint64_t* mbar = reinterpret_cast<uint64_t*>(zt + C::ZR * CM_ZTAB_W);
 
   const int t = threadIdx.x;
@@ -335,12 +338,13 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
 #pragma unroll
       for (int v = 0; v < NV; ++v) cm7_bulk_g2s(Rt + v * SLOT, p.dQ + v * p.stride + src, SLOT * 8, mbar);
   }
-  cm7_prefetch_traces<Nq, NV, SGS ? C::NGD : 0, NT, THREADS>(p, pos, t, T, zt);
+  cm7_prefetch_traces<Nq, NV, SGS ? C::NGD : 0, TS, THREADS>(p, pos, t, T, zt);
 
   double* Qs = Qt + sh; double* Fs = Ft + sh; double* cs = ct + sh; const double* Rs = Rt + sh;
   const int n = t;
   const bool node = t < NP;
   const int k_ = n / NF, j_ = (n - k_ * NF) / Nq, i_ = n - k_ * NF - j_ * Nq;
+  const int nT = j_ + Nq * i_ + NF * k_;               // index in the F^2 tiles (i, j swapped)
   cm7_cp_wait_but_one();                               // this thread's z-row copies have landed
   __syncthreads();                                     // mbarrier init and z rows visible
   cm7_mbar_wait(mbar, 0);
@@ -363,7 +367,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
     cm_flux_axis<MOIST, 1>(Y, P, SGS, g, p.cA[1], Fb);
     cm_flux_axis<MOIST, 2>(Y, P, SGS, g, p.cA[2], Fc);
 #pragma unroll
-    for (int v = 0; v < NV; ++v) { Fs[v * SLOT + n] = Fa[v]; Fs[(NV + v) * SLOT + n] = Fb[v]; Fs[(2 * NV + v) * SLOT + n] = Fc[v]; }
+    for (int v = 0; v < NV; ++v) { Fs[v * SLOT + n] = Fa[v]; Fs[(NV + v) * SLOT + n] = Fc[v]; Fs[(2 * NV + v) * SLOT + nT] = Fb[v]; }
   }
   cm7_cp_wait_all();                                   // this thread's trace copies have landed
   __syncthreads();                                     // fluxes, sound speed and everybody's traces visible
@@ -374,8 +378,8 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
     const int d = lt / NFP, l = lt % NFP;
     if (l < NF) {
       if (d == 0) cm7_tend_line<Nq, MOIST, 0>(p, Fs, pos.wallmask, l);
-      else if (d == 1) cm7_tend_line<Nq, MOIST, 1>(p, Fs + NV * SLOT, pos.wallmask, l);
-      else cm7_tend_line<Nq, MOIST, 2>(p, Fs + 2 * NV * SLOT, pos.wallmask, l);
+      else if (d == 1) cm7_tend_line<Nq, MOIST, 1>(p, Fs + 2 * NV * SLOT, pos.wallmask, l);
+      else cm7_tend_line<Nq, MOIST, 2>(p, Fs + NV * SLOT, pos.wallmask, l);
     }
   }
   __syncthreads();
@@ -385,7 +389,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
     double acc[6], lift[6], Yo[6], Ro[6];
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
-      acc[v] = Fs[v * SLOT + n] + Fs[(NV + v) * SLOT + n] + Fs[(2 * NV + v) * SLOT + n];
+      acc[v] = Fs[v * SLOT + n] + Fs[(2 * NV + v) * SLOT + nT] + Fs[(NV + v) * SLOT + n];
       lift[v] = 0.0;
       if (MODE != 0) Yo[v] = Qs[v * SLOT + n];
       if (MODE == 1) Ro[v] = Rs[v * SLOT + n];
@@ -396,7 +400,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
 #pragma unroll
     for (int d = 0; d < 3; ++d)
       if (c3[d] == 0 || c3[d] == N) {
-        const double* tr = T + (2 * d + (c3[d] == N ? 1 : 0)) * (NT * NF) + m3[d];
+        const double* tr = T + (2 * d + (c3[d] == N ? 1 : 0)) * TS + m3[d];
 #pragma unroll
         for (int v = 0; v < NV; ++v) lift[v] += tr[v * NF];
       }
@@ -429,10 +433,10 @@ template <int Nq, bool MOIST>
 __device__ __forceinline__ void cm7_grad_face(const CmKP& p, const double* __restrict__ ss, double* __restrict__ T,
                                               const double* __restrict__ zt, int wallmask, int fn) {
   using C = CmCfg7<Nq, MOIST>;
-  constexpr int NF = C::NF, NV = C::NV, NS = C::NS, SLOT = C::SLOT;
+  constexpr int NF = C::NF, NV = C::NV, NS = C::NS, SLOT = C::SLOT, TS = C::TS_G;
   int f, m, d, s, nm, np_, kline;
   cm7_face_node<Nq>(fn, f, m, d, s, nm, np_, kline);
-  double* tr = T + f * (NV * NF) + m;
+  double* tr = T + f * TS + m;
   double dl[5];
   if (!((wallmask >> f) & 1)) {
     double Yp[6], sp[5];
@@ -453,13 +457,14 @@ __device__ __forceinline__ void cm7_grad_face(const CmKP& p, const double* __res
 template <int Nq, bool MOIST, int D>
 __device__ __forceinline__ void cm7_grad_line(const CmKP& p, const double* __restrict__ ss, double* __restrict__ dd, int l) {
   using C = CmCfg7<Nq, MOIST>;
-  constexpr int NF = C::NF, NS = C::NS, SLOT = C::SLOT, STR = Cm7Str<Nq, D>::value;
+  constexpr int NF = C::NF, NS = C::NS, SLOT = C::SLOT, STR = Cm7Str<Nq, D>::value, OSTR = (D == 2) ? NF : 1;
   const int b = l / Nq, a = l - b * Nq;
   const int base = (D == 0) ? Nq * l : (D == 1) ? a + NF * b : l;
+  const int obase = (D == 2) ? l : Nq * l;              // eta-derivatives are stored with i and j swapped (contiguous)
 #pragma unroll
   for (int v = 0; v < NS; ++v) {
     const double* in = ss + v * SLOT + base;
-    double* out = dd + v * SLOT + base;
+    double* out = dd + v * SLOT + obase;
     double x[Nq];
 #pragma unroll
     for (int m = 0; m < Nq; ++m) x[m] = in[m * STR];
@@ -468,7 +473,7 @@ __device__ __forceinline__ void cm7_grad_line(const CmKP& p, const double* __res
       double s = 0.0;
 #pragma unroll
       for (int m = 0; m < Nq; ++m) s += p.D[i][m] * x[m];
-      out[i * STR] = s;
+      out[i * OSTR] = s;
     }
   }
 }
@@ -478,11 +483,12 @@ template <int Nq, bool MOIST, bool RAW>
 __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>::MINB_G) cm7_gradient_kernel(const __grid_constant__ CmKP p) {
   using C = CmCfg7<Nq, MOIST>;
   constexpr int NF = C::NF, NP = C::NP, N = Nq - 1, NV = C::NV, NS = C::NS, SLOT = C::SLOT, NFP = C::NFP, THREADS = C::THREADS;
+  constexpr int TS = C::TS_G;
   extern __shared__ __align__(128) double smem7[];
   double* Qt = smem7;                                  // [NV][SLOT]      state, then the gradient variables in place
   double* dt_ = Qt + NV * SLOT;                        // [3][NS][SLOT]   reference-space derivatives
-  double* T = dt_ + 3 * NS * SLOT;                     // [6][NV][NF]     neighbour traces, then s* - s^-
-  double* zt = T + 6 * NV * NF;                        // [ZR][CM_ZTAB_W]
+  double* T = dt_ + 3 * NS * SLOT;                     // [6][TS]         neighbour traces [v][m] per face, then s* - s^-
+  double* zt = T + 6 * TS;                        // [ZR][CM_ZTAB_W]
   uint64_t* mbar = reinterpret_cast<uint64_t*>(zt + C::ZR * CM_ZTAB_W);
 
   const int t = threadIdx.x;
@@ -497,11 +503,12 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
 #pragma unroll
     for (int v = 0; v < NV; ++v) cm7_bulk_g2s(Qt + v * SLOT, p.Q + v * p.stride + src, SLOT * 8, mbar);
   }
-  cm7_prefetch_traces<Nq, NV, 0, NV, THREADS>(p, pos, t, T, zt);
+  cm7_prefetch_traces<Nq, NV, 0, TS, THREADS>(p, pos, t, T, zt);
   double* ss = Qt + sh; double* dd = dt_ + sh;
   const int n = t;
   const bool node = t < NP;
   const int k_ = n / NF, j_ = (n - k_ * NF) / Nq, i_ = n - k_ * NF - j_ * Nq;
+  const int nT = j_ + Nq * i_ + NF * k_;               // index in the eta-derivative tiles (i, j swapped)
   cm7_cp_wait_but_one();
   __syncthreads();
   cm7_mbar_wait(mbar, 0);
@@ -539,10 +546,10 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
 #pragma unroll
-      for (int v = 0; v < NS; ++v) Gr[v][c] = dd[(c * NS + v) * SLOT + n];
+      for (int v = 0; v < NS; ++v) Gr[v][c] = dd[(c * NS + v) * SLOT + (c == 1 ? nT : n)];
       if (c3[c] == 0 || c3[c] == N) {
         const bool hi = (c3[c] == N);
-        const double* tr = T + (2 * c + (hi ? 1 : 0)) * (NV * NF) + m3[c];
+        const double* tr = T + (2 * c + (hi ? 1 : 0)) * TS + m3[c];
         const double w = hi ? p.inv_w0 : -p.inv_w0;
 #pragma unroll
         for (int v = 0; v < NS; ++v) Gr[v][c] += w * tr[v * NF];
