@@ -579,3 +579,188 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
     }
   }
 }
+
+// ------------------------------------------------------------------------------------------------
+// a2, second form (used when every line task has its own thread, 3 * NFP <= THREADS): the line task owns the face
+// terms of its two end nodes.  Its 2 x NV neighbour-trace values are loaded into REGISTERS at CTA start (the addresses
+// follow from blockIdx, so the loads are in flight together with the bulk TMA of the element's own tiles) and are
+// consumed only in phase 2: no trace buffer, no cp.async, no second pass over the face nodes, and the lifted jumps
+// are folded into the line's end values -- half the shared-memory traffic of cm7_gradient_kernel (profiles/r1d_v7.md:
+// that kernel kept the shared-memory data pipe 78 % busy).
+// ------------------------------------------------------------------------------------------------
+template <int Nq, bool MOIST> struct CmCfg9 {
+  using C7 = CmCfg7<Nq, MOIST>;
+  static constexpr int GRAD_DOUBLES = (C7::NV + 3 * C7::NS) * C7::SLOT + 2;   // Q (then s in place), ds/dxi_d, mbarrier
+  static constexpr size_t GRAD_SMEM = sizeof(double) * GRAD_DOUBLES;
+  static constexpr bool OK = 3 * C7::NFP <= C7::THREADS;
+  static constexpr int MINB_G = C7::cap(C7::fit(GRAD_SMEM), C7::cap(896 / C7::THREADS, 16));
+};
+
+// line l of direction D -> first node and zeta index.  For Nq = 5 the eta-lines are dealt to the lanes so that each
+// half-warp holds whole zeta-planes {0, 1, 4} and {2, 3}: the 25-double plane stride then costs one 2-way bank
+// conflict instead of two (lanes 15 and 26..31 idle).
+template <int Nq, int D>
+__device__ __forceinline__ bool cm9_line(int l, int& base, int& kline) {
+  constexpr int NF = Nq * Nq;
+  if (D == 1 && Nq == 5) {
+    int a, b;
+    if (l < 10) { b = l / 5; a = l - 5 * b; }
+    else if (l < 15) { b = 4; a = l - 10; }
+    else if (l >= 16 && l < 26) { b = 2 + (l - 16) / 5; a = (l - 16) % 5; }
+    else return false;
+    base = a + NF * b; kline = b;
+    return true;
+  }
+  if (l >= NF) return false;
+  const int b = l / Nq, a = l - b * Nq;
+  base = (D == 0) ? Nq * l : (D == 1) ? a + NF * b : l;
+  kline = b;
+  return true;
+}
+
+template <int Nq, bool MOIST, int D>
+__device__ __forceinline__ void cm9_grad_line(const CmKP& p, const double* __restrict__ ss, double* __restrict__ dd,
+                                              const double (&Yp)[2][6], const double (&Php)[2], int wallmask, int base) {
+  using C = CmCfg7<Nq, MOIST>;
+  constexpr int N = Nq - 1, NS = C::NS, SLOT = C::SLOT, STR = Cm7Str<Nq, D>::value;
+  double dl[2][5];                                      // s* - s^- at the two ends (eq. 30-31: central flux)
+#pragma unroll
+  for (int s = 0; s < 2; ++s) {
+    const int nm = s ? base + N * STR : base;
+    if (!((wallmask >> (2 * D + s)) & 1)) {
+      double sp[5];
+      cm7_eos_grad<MOIST>(p, Yp[s], Php[s], sp);
+#pragma unroll
+      for (int v = 0; v < NS; ++v) dl[s][v] = 0.5 * (sp[v] - ss[v * SLOT + nm]);
+    } else {
+      // wall: u_bc = u^- - (n.u^-) n  (A6); scalars unchanged (A8)
+#pragma unroll
+      for (int v = 0; v < NS; ++v) dl[s][v] = (v == D) ? -ss[v * SLOT + nm] : 0.0;
+    }
+  }
+#pragma unroll
+  for (int v = 0; v < NS; ++v) {
+    const double* in = ss + v * SLOT + base;
+    double* out = dd + v * SLOT + base;
+    double x[Nq];
+#pragma unroll
+    for (int m = 0; m < Nq; ++m) x[m] = in[m * STR];
+#pragma unroll
+    for (int i = 0; i < Nq; ++i) {
+      double a = 0.0;
+#pragma unroll
+      for (int m = 0; m < Nq; ++m) a += p.D[i][m] * x[m];
+      if (i == 0) a -= p.inv_w0 * dl[0][v];
+      if (i == N) a += p.inv_w0 * dl[1][v];
+      out[i * STR] = a;
+    }
+  }
+}
+
+template <int Nq, bool MOIST, bool RAW>
+__global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg9<Nq, MOIST>::MINB_G) cm9_gradient_kernel(const __grid_constant__ CmKP p) {
+  using C = CmCfg7<Nq, MOIST>;
+  constexpr int NF = C::NF, NP = C::NP, N = Nq - 1, NV = C::NV, NS = C::NS, SLOT = C::SLOT, NFP = C::NFP, THREADS = C::THREADS;
+  extern __shared__ __align__(128) double smem7[];
+  double* Qt = smem7;                                  // [NV][SLOT]      state, then the gradient variables in place
+  double* dt_ = Qt + NV * SLOT;                        // [3][NS][SLOT]   reference-space derivatives + lifted jumps
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(dt_ + 3 * NS * SLOT);
+
+  const int t = threadIdx.x;
+  const Cm7Pos pos = cm7_position(p);
+  const int e = pos.e;
+  const int sh = C::ODD ? (e & 1) : 0;
+  if (t == THREADS - 32) {
+    cm7_mbar_init(mbar, 1);
+    cm7_fence_mbar_init();
+    const long long src = (long long)e * NP - sh;
+    cm7_mbar_expect_tx(mbar, (uint32_t)(NV * SLOT * sizeof(double)));
+#pragma unroll
+    for (int v = 0; v < NV; ++v) cm7_bulk_g2s(Qt + v * SLOT, p.Q + v * p.stride + src, SLOT * 8, mbar);
+  }
+
+  // ---- the thread's line task and the neighbour traces of its two end nodes, into registers
+  const int d = t / NFP, l = t - d * NFP;
+  int base = 0, kline = 0;
+  bool line = false;
+  if (d == 0) line = cm9_line<Nq, 0>(l, base, kline);
+  else if (d == 1) line = cm9_line<Nq, 1>(l, base, kline);
+  else if (d == 2) line = cm9_line<Nq, 2>(l, base, kline);
+  double Yp[2][6], Php[2];
+#pragma unroll
+  for (int s = 0; s < 2; ++s) {
+#pragma unroll
+    for (int v = 0; v < 6; ++v) Yp[s][v] = 1.0;
+    Php[s] = 0.0;
+  }
+  if (line) {
+    const int span = N * ((d == 0) ? 1 : (d == 1) ? Nq : NF);
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+      if (!((pos.wallmask >> (2 * d + s)) & 1)) {
+        const double* src = p.Q + (size_t)cm7_neighbour(p, pos, d, s) * NP + (s ? base : base + span);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) { Yp[s][v] = __ldg(src); src += p.stride; }
+        int row = pos.ez * Nq + kline;                                   // d < 2: the neighbour node is at the same height
+        if (d == 2) row = s ? ((pos.ez + 1 == p.gEz) ? 0 : (pos.ez + 1) * Nq) : ((pos.ez == 0 ? p.gEz : pos.ez) * Nq - 1);
+        Php[s] = __ldg(p.ztab + (size_t)row * CM_ZTAB_W);
+      }
+  }
+
+  double* ss = Qt + sh; double* dd = dt_ + sh;
+  const int n = t;
+  const bool node = t < NP;
+  double Phi = 0.0;
+  if (node) Phi = __ldg(p.ztab + (size_t)(pos.ez * Nq + n / NF) * CM_ZTAB_W);
+  __syncthreads();                                     // mbarrier init visible
+  cm7_mbar_wait(mbar, 0);
+
+  // ---- phase 1: gradient variables of the own node, in place of the state
+  if (node) {
+    double Y[6], s[5];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) Y[v] = ss[v * SLOT + n];
+    cm7_eos_grad<MOIST>(p, Y, Phi, s);
+#pragma unroll
+    for (int v = 0; v < NS; ++v) ss[v * SLOT + n] = s[v];
+  }
+  __syncthreads();
+
+  // ---- phase 2: one thread per line: contraction + lifted jumps at its two ends
+  if (line) {
+    if (d == 0) cm9_grad_line<Nq, MOIST, 0>(p, ss, dd, Yp, Php, pos.wallmask, base);
+    else if (d == 1) cm9_grad_line<Nq, MOIST, 1>(p, ss, dd + NS * SLOT, Yp, Php, pos.wallmask, base);
+    else cm9_grad_line<Nq, MOIST, 2>(p, ss, dd + 2 * NS * SLOT, Yp, Php, pos.wallmask, base);
+  }
+  __syncthreads();
+
+  // ---- phase 3: physical gradient, closure, store
+  if (node) {
+    const size_t idx = (size_t)e * NP + n;
+    double Gr[5][3];
+#pragma unroll
+    for (int v = 0; v < NS; ++v)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) Gr[v][c] = (p.cA[c] * p.invJ) * dd[(c * NS + v) * SLOT + n];
+    if (!MOIST) { Gr[4][0] = Gr[4][1] = Gr[4][2] = 0.0; }
+    double* o = p.Gout + idx;
+    const long long st = p.stride;
+    if (RAW) {
+#pragma unroll
+      for (int v = 0; v < 5; ++v)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) __stcs(o + (size_t)(3 * v + c) * st, Gr[v][c]);
+    } else {
+      // eq. (33)-(38): S, nu_t = (C_s Delta)^2 sqrt(2 S:S), D_t = nu_t / Pr_t; store tau, J + D, d_q
+      const double Sxx = Gr[0][0], Syy = Gr[1][1], Szz = Gr[2][2];
+      const double Sxy = 0.5 * (Gr[0][1] + Gr[1][0]), Sxz = 0.5 * (Gr[0][2] + Gr[2][0]), Syz = 0.5 * (Gr[1][2] + Gr[2][1]);
+      const double ss2 = Sxx * Sxx + Syy * Syy + Szz * Szz + 2.0 * (Sxy * Sxy + Sxz * Sxz + Syz * Syz);
+      const double nu = p.cs2delta2 * cm_sqrt(2.0 * ss2);
+      const double m2nu = -2.0 * nu, mDt = -nu * p.inv_Pr;
+      o[0] = m2nu * Sxx; o[st] = m2nu * Syy; o[2 * st] = m2nu * Szz;
+      o[3 * st] = m2nu * Sxy; o[4 * st] = m2nu * Sxz; o[5 * st] = m2nu * Syz;
+      o[6 * st] = mDt * Gr[3][0]; o[7 * st] = mDt * Gr[3][1]; o[8 * st] = mDt * Gr[3][2];
+      if (MOIST) { o[9 * st] = mDt * Gr[4][0]; o[10 * st] = mDt * Gr[4][1]; o[11 * st] = mDt * Gr[4][2]; }
+    }
+  }
+}

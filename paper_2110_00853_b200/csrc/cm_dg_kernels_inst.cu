@@ -63,9 +63,18 @@ template <int Nq, bool MOIST, bool RAW>
 cudaError_t launch_grad7(const CmKP& kp, cudaStream_t st) {
   using C = CmCfg7<Nq, MOIST>;
   static bool configured = false;
-  cudaError_t err = configure(cm7_gradient_kernel<Nq, MOIST, RAW>, C::GRAD_SMEM, configured);
-  if (err != cudaSuccess) return err;
-  cm7_gradient_kernel<Nq, MOIST, RAW><<<dim3(kp.gPY * kp.gL, kp.gEz, kp.gNXC * kp.gNYP), C::THREADS, C::GRAD_SMEM, st>>>(kp);
+  const dim3 grid(kp.gPY * kp.gL, kp.gEz, kp.gNXC * kp.gNYP);
+  if constexpr (CmCfg9<Nq, MOIST>::OK) {
+    // every line task has its own thread: register-staged traces (cm9_gradient_kernel)
+    constexpr size_t smem = CmCfg9<Nq, MOIST>::GRAD_SMEM;
+    cudaError_t err = configure(cm9_gradient_kernel<Nq, MOIST, RAW>, smem, configured);
+    if (err != cudaSuccess) return err;
+    cm9_gradient_kernel<Nq, MOIST, RAW><<<grid, C::THREADS, smem, st>>>(kp);
+  } else {
+    cudaError_t err = configure(cm7_gradient_kernel<Nq, MOIST, RAW>, C::GRAD_SMEM, configured);
+    if (err != cudaSuccess) return err;
+    cm7_gradient_kernel<Nq, MOIST, RAW><<<grid, C::THREADS, C::GRAD_SMEM, st>>>(kp);
+  }
   return cudaGetLastError();
 }
 
