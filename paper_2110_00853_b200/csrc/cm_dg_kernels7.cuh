@@ -57,6 +57,8 @@ __device__ __forceinline__ void cm7_cp_commit() { asm volatile("cp.async.commit_
 __device__ __forceinline__ void cm7_cp_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void cm7_cp_wait_but_one() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 
+#define CM_ZSM_W 10   // doubles per z-table row in shared memory (CmCfg7::ZW)
+
 template <int Nq, bool MOIST> struct CmCfg7 {
   static constexpr int NF = Nq * Nq;
   static constexpr int NP = Nq * Nq * Nq;
@@ -70,13 +72,18 @@ template <int Nq, bool MOIST> struct CmCfg7 {
   static constexpr int THREADS = ((NP + 31) / 32) * 32;
   static constexpr int NFP = ((NF + 31) / 32) * 32;         // line tasks of one direction, padded to whole warps
   static constexpr int ZR = Nq + 2;                         // z-table rows: facing row below, own Nq rows, facing row above
-  static constexpr int TAIL = ZR * CM_ZTAB_W + 2;           // z rows, mbarrier
+  static constexpr int ZW = 10;                             // doubles per z row in shared memory: rows fall into disjoint banks
+  static constexpr int TAIL = (ZR - 1) * ZW + 7 + 1;        // z rows (7 values used per row), mbarrier
   // stride between the trace blocks of two faces: >= rows * NF and = NF (mod 16), so that consecutive face nodes of a
   // warp that straddles two faces fall into consecutive banks
   static constexpr int fstride(int rows) { return rows * NF + ((NF - rows * NF) % 16 + 16) % 16; }
   static constexpr int TS_T = fstride(NTR), TS_G = fstride(NV);
-  static constexpr int TEND_DOUBLES = (NV + 3 * NV + 1 + NV) * SLOT + 6 * TS_T + TAIL;   // Q, F^1 F^3 F^2 (G lands in F^1,F^3), c, residual, traces
-  static constexpr int GRAD_DOUBLES = (NV + 3 * NS) * SLOT + 6 * TS_G + TAIL;            // Q (then s in place), ds/dxi_d, traces
+  // F^2 tiles (tendency): node (i, j, k) at i + Nq j + PS2 k.  At Nq = 5 a zeta-plane stride of 27 puts the 15 / 10
+  // eta-lines of zeta-planes {0,1,2} / {3,4} into distinct banks (cm7_yline deals the lines to the lanes that way)
+  static constexpr int PS2 = (Nq == 5) ? NF + 2 : NF;
+  static constexpr int SLOT2 = (Nq - 1) * PS2 + NF;
+  static constexpr int TEND_DOUBLES = (NV + 2 * NV + 1 + NV) * SLOT + NV * SLOT2 + 5 * TS_T + NTR * NF + TAIL;   // Q, F^1 F^3 (G lands there), c, residual, F^2, traces
+  static constexpr int GRAD_DOUBLES = (NV + 3 * NS) * SLOT + 5 * TS_G + NV * NF + TAIL;            // Q (then s in place), ds/dxi_d, traces
   static_assert(2 * NV >= NG, "the packed SGS fluxes are staged in the F^1, F^3 tiles");
   static constexpr size_t TEND_SMEM = sizeof(double) * TEND_DOUBLES;
   static constexpr size_t GRAD_SMEM = sizeof(double) * GRAD_DOUBLES;
@@ -177,12 +184,12 @@ __device__ __forceinline__ void cm7_prefetch_traces(const CmKP& p, const Cm7Pos&
                                                     double* __restrict__ zt) {
   constexpr int NF = Nq * Nq, NP = NF * Nq, ZR = Nq + 2;
   // group 0: z rows (phase 1 needs them)
-  for (int c = t; c < ZR * CM_ZTAB_W; c += THREADS) {
-    const int r = c / CM_ZTAB_W;
+  for (int c = t; c < ZR * 7; c += THREADS) {
+    const int r = c / 7, col = c - 7 * r;
     int row = q.ez * Nq + r - 1;                                           // own rows; r = 0 / ZR-1: the facing rows below / above
     if (r == 0) row = (q.wallmask & 16) ? -1 : (q.ez > 0 ? row : p.gEz * Nq - 1);
     if (r == ZR - 1) row = (q.wallmask & 32) ? -1 : (q.ez < p.gEz - 1 ? row : 0);
-    if (row >= 0) cm7_cp8(zt + c, p.ztab + (size_t)row * CM_ZTAB_W + (c % CM_ZTAB_W));
+    if (row >= 0) cm7_cp8(zt + r * CM_ZSM_W + col, p.ztab + (size_t)row * CM_ZTAB_W + col);
   }
   cm7_cp_commit();
   // group 1: neighbour traces (phase 2 needs them)
@@ -239,7 +246,7 @@ __device__ __forceinline__ void cm7_tend_face(const CmKP& p, const double* __res
     if (SGS)
 #pragma unroll
       for (int k = 0; k < NGD; ++k) gp[k] = tr[(NV + k) * NF];
-    cm7_site(zt + ((d < 2) ? 1 + kline : (s ? Nq + 1 : 0)) * CM_ZTAB_W, st);
+    cm7_site(zt + ((d < 2) ? 1 + kline : (s ? Nq + 1 : 0)) * CM_ZSM_W, st);
     cm_eos<MOIST>(p, Yp, st, P);
     const double ud = (d == 0) ? P.u : (d == 1) ? P.v : P.w;
     double wA = ud, t0 = 0.0, t1 = 0.0, t2 = 0.0, eA = 0.0, dqA = 0.0;
@@ -261,7 +268,7 @@ __device__ __forceinline__ void cm7_tend_face(const CmKP& p, const double* __res
 #pragma unroll
     for (int v = 0; v < NV; ++v) rf[v] = hA * Fp[v] + hl * (Ym[v] - Yp[v]);
   } else {
-    cm7_site(zt + ((d < 2) ? 1 + kline : (s ? Nq : 1)) * CM_ZTAB_W, st);
+    cm7_site(zt + ((d < 2) ? 1 + kline : (s ? Nq : 1)) * CM_ZSM_W, st);
     cm_eos<MOIST>(p, Ym, st, P);
     const double lam = fabs(unm) + cm_;
     const double mom = -(P.pp + Ym[0] * unm * (unm + lam)) * A;
@@ -274,19 +281,35 @@ __device__ __forceinline__ void cm7_tend_face(const CmKP& p, const double* __res
   for (int v = 0; v < NV; ++v) tr[v * NF] = rf[v];
 }
 
-// tendency, phase 2b: line task.  Fd = the NV tiles holding F^D (F^2 tiles are stored with i and j swapped, so the
-// eta-lines are contiguous like the xi-lines: no bank conflicts in any direction); on return the line holds D_D F^D minus the lifted
-// own-side half of the face term at its two ends (eq. 32)
-template <int Nq, bool MOIST, int D>
-__device__ __forceinline__ void cm7_tend_line(const CmKP& p, double* __restrict__ Fd, int wallmask, int l) {
-  using C = CmCfg7<Nq, MOIST>;
-  constexpr int N = Nq - 1, NV = C::NV, SLOT = C::SLOT, STR = (D == 2) ? Nq * Nq : 1;   // F^2 tiles: i, j swapped
-  const int base = (D == 2) ? l : Nq * l;
+// eta-line l -> first node in an F^2 tile; false = idle lane.  Nq = 5: lanes 0..14 hold zeta-planes 0..2, lanes 16..25
+// planes 3..4 (see CmCfg7::PS2)
+template <int Nq>
+__device__ __forceinline__ bool cm7_yline(int l, int& base) {
+  constexpr int NF = Nq * Nq, PS2 = (Nq == 5) ? NF + 2 : NF;
+  if (Nq == 5) {
+    if (l == 15 || l >= 26) return false;
+    const int ll = (l < 15) ? l : l - 1;              // 0..24
+    const int b = ll / 5, a = ll - 5 * b;
+    base = a + PS2 * b;
+    return true;
+  }
+  if (l >= NF) return false;
+  const int b = l / Nq, a = l - b * Nq;
+  base = a + PS2 * b;
+  return true;
+}
+
+// tendency, phase 2b: line task.  q0 = first node of the line in the first of the NV tiles holding F^D (tile stride
+// TSL, node stride STR); on return the line holds D_D F^D minus the lifted own-side half of the face term at its two
+// ends (eq. 32)
+template <int Nq, int NV, int TSL, int STR, int D>
+__device__ __forceinline__ void cm7_tend_line(const CmKP& p, double* __restrict__ q0, int wallmask) {
+  constexpr int N = Nq - 1;
   const double c0 = p.inv_w0 * (((wallmask >> (2 * D)) & 1) ? 1.0 : 0.5);      // -sgn = +1 at the low end
   const double cN = -p.inv_w0 * (((wallmask >> (2 * D + 1)) & 1) ? 1.0 : 0.5);
 #pragma unroll
   for (int v = 0; v < NV; ++v) {
-    double* q = Fd + v * SLOT + base;
+    double* q = q0 + v * TSL;
     double x[Nq], y[Nq];
 #pragma unroll
     for (int m = 0; m < Nq; ++m) x[m] = q[m * STR];
@@ -312,12 +335,13 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
   constexpr int TS = C::TS_T;
   extern __shared__ __align__(128) double smem7[];
   double* Qt = smem7;                                  // [NV][SLOT]     state
-  double* Ft = Qt + NV * SLOT;                         // [3][NV][SLOT]  F^1, F^3 (the packed SGS fluxes G land here), F^2 (i, j swapped)
-  double* ct = Ft + 3 * NV * SLOT;                     // [SLOT]         sound speed
+  double* Ft = Qt + NV * SLOT;                         // [2][NV][SLOT]  F^1, F^3 (the packed SGS fluxes G land here)
+  double* ct = Ft + 2 * NV * SLOT;                     // [SLOT]         sound speed
   double* Rt = ct + SLOT;                              // [NV][SLOT]     LSRK residual
-  double* T = Rt + NV * SLOT;                          // [6][TS]        neighbour traces [v][m] per face, then rf
-  double* zt = T + 6 * TS;                    // [ZR][CM_ZTAB_W]
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(zt + C::ZR * CM_ZTAB_W);
+  double* F2 = Rt + NV * SLOT;                         // [NV][SLOT2]    F^2 (zeta-plane stride PS2)
+  double* T = F2 + NV * C::SLOT2;                          // [6][TS]        neighbour traces [v][m] per face, then rf
+  double* zt = T + 5 * TS + C::NTR * NF;      // [ZR][CM_ZSM_W]
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(zt + (C::ZR - 1) * CM_ZSM_W + 7);
 
   const int t = threadIdx.x;
   const Cm7Pos pos = cm7_position(p);
@@ -344,7 +368,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
   const int n = t;
   const bool node = t < NP;
   const int k_ = n / NF, j_ = (n - k_ * NF) / Nq, i_ = n - k_ * NF - j_ * Nq;
-  const int nT = j_ + Nq * i_ + NF * k_;               // index in the F^2 tiles (i, j swapped)
+  const int n2 = n + (C::PS2 - NF) * k_;               // index in the F^2 tiles
   cm7_cp_wait_but_one();                               // this thread's z-row copies have landed
   __syncthreads();                                     // mbarrier init and z rows visible
   cm7_mbar_wait(mbar, 0);
@@ -353,7 +377,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
   double buoy = 0.0;
   if (node) {
     double Y[6], g[12]; CmPrim P; CmSite st;
-    cm7_site(zt + (1 + k_) * CM_ZTAB_W, st);
+    cm7_site(zt + (1 + k_) * CM_ZSM_W, st);
 #pragma unroll
     for (int v = 0; v < NV; ++v) Y[v] = Qs[v * SLOT + n];
     if (SGS)
@@ -367,7 +391,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
     cm_flux_axis<MOIST, 1>(Y, P, SGS, g, p.cA[1], Fb);
     cm_flux_axis<MOIST, 2>(Y, P, SGS, g, p.cA[2], Fc);
 #pragma unroll
-    for (int v = 0; v < NV; ++v) { Fs[v * SLOT + n] = Fa[v]; Fs[(NV + v) * SLOT + n] = Fc[v]; Fs[(2 * NV + v) * SLOT + nT] = Fb[v]; }
+    for (int v = 0; v < NV; ++v) { Fs[v * SLOT + n] = Fa[v]; Fs[(NV + v) * SLOT + n] = Fc[v]; F2[v * C::SLOT2 + n2] = Fb[v]; }
   }
   cm7_cp_wait_all();                                   // this thread's trace copies have landed
   __syncthreads();                                     // fluxes, sound speed and everybody's traces visible
@@ -376,11 +400,9 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
   for (int fn = THREADS - 1 - t; fn < 6 * NF; fn += THREADS) cm7_tend_face<Nq, MOIST, SGS>(p, Qs, cs, T, zt, pos.wallmask, fn);
   for (int lt = t; lt < 3 * NFP; lt += THREADS) {
     const int d = lt / NFP, l = lt % NFP;
-    if (l < NF) {
-      if (d == 0) cm7_tend_line<Nq, MOIST, 0>(p, Fs, pos.wallmask, l);
-      else if (d == 1) cm7_tend_line<Nq, MOIST, 1>(p, Fs + 2 * NV * SLOT, pos.wallmask, l);
-      else cm7_tend_line<Nq, MOIST, 2>(p, Fs + NV * SLOT, pos.wallmask, l);
-    }
+    if (d == 0) { if (l < NF) cm7_tend_line<Nq, NV, SLOT, 1, 0>(p, Fs + Nq * l, pos.wallmask); }
+    else if (d == 1) { int base; if (cm7_yline<Nq>(l, base)) cm7_tend_line<Nq, NV, C::SLOT2, Nq, 1>(p, F2 + base, pos.wallmask); }
+    else { if (l < NF) cm7_tend_line<Nq, NV, SLOT, NF, 2>(p, Fs + NV * SLOT + l, pos.wallmask); }
   }
   __syncthreads();
 
@@ -389,7 +411,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
     double acc[6], lift[6], Yo[6], Ro[6];
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
-      acc[v] = Fs[v * SLOT + n] + Fs[(2 * NV + v) * SLOT + nT] + Fs[(NV + v) * SLOT + n];
+      acc[v] = Fs[v * SLOT + n] + F2[v * C::SLOT2 + n2] + Fs[(NV + v) * SLOT + n];
       lift[v] = 0.0;
       if (MODE != 0) Yo[v] = Qs[v * SLOT + n];
       if (MODE == 1) Ro[v] = Rs[v * SLOT + n];
@@ -442,7 +464,7 @@ __device__ __forceinline__ void cm7_grad_face(const CmKP& p, const double* __res
     double Yp[6], sp[5];
 #pragma unroll
     for (int v = 0; v < NV; ++v) Yp[v] = tr[v * NF];
-    cm7_eos_grad<MOIST>(p, Yp, zt[((d < 2) ? 1 + kline : (s ? Nq + 1 : 0)) * CM_ZTAB_W], sp);
+    cm7_eos_grad<MOIST>(p, Yp, zt[((d < 2) ? 1 + kline : (s ? Nq + 1 : 0)) * CM_ZSM_W], sp);
 #pragma unroll
     for (int v = 0; v < NS; ++v) dl[v] = 0.5 * (sp[v] - ss[v * SLOT + nm]);
   } else {
@@ -488,8 +510,8 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
   double* Qt = smem7;                                  // [NV][SLOT]      state, then the gradient variables in place
   double* dt_ = Qt + NV * SLOT;                        // [3][NS][SLOT]   reference-space derivatives
   double* T = dt_ + 3 * NS * SLOT;                     // [6][TS]         neighbour traces [v][m] per face, then s* - s^-
-  double* zt = T + 6 * TS;                        // [ZR][CM_ZTAB_W]
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(zt + C::ZR * CM_ZTAB_W);
+  double* zt = T + 5 * TS + NV * NF;              // [ZR][CM_ZSM_W]
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(zt + (C::ZR - 1) * CM_ZSM_W + 7);
 
   const int t = threadIdx.x;
   const Cm7Pos pos = cm7_position(p);
@@ -518,7 +540,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
     double Y[6], s[5];
 #pragma unroll
     for (int v = 0; v < NV; ++v) Y[v] = ss[v * SLOT + n];
-    cm7_eos_grad<MOIST>(p, Y, zt[(1 + k_) * CM_ZTAB_W], s);
+    cm7_eos_grad<MOIST>(p, Y, zt[(1 + k_) * CM_ZSM_W], s);
 #pragma unroll
     for (int v = 0; v < NS; ++v) ss[v * SLOT + n] = s[v];
   }
