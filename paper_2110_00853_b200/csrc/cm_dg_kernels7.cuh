@@ -1,26 +1,33 @@
 // cm_dg_kernels7.cuh -- the hot kernels for flat bricks (GEOM == 0): one small CTA per element, every input staged
-// asynchronously into shared memory at CTA start, face work and line work decoupled so that all warps stay busy.
+// asynchronously at CTA start, face work and line work decoupled so that all warps stay busy.
 //
-// Lessons built in (profiles/r1c_v5.md, profiles/r1d_v6.md): the kernels are bound by instruction latency at ~20
-// resident warps per SM (shared memory holds five elements per SM), so what counts is the length of the dependent
-// instruction chain of each warp and that no warp idles at a barrier:
-//   * CTA start: lane 0 of the last warp fetches the element's own Q, packed SGS fluxes G and LSRK residual by 1-D
-//     bulk TMA (cp.async.bulk ... mbarrier::complete_tx); every thread copies the neighbour traces of one or two face
-//     nodes (6 state values + the 5 SGS values the face-normal flux needs) and the z-table rows with 8-byte cp.async.
-//     Element position, neighbour ids, wall flags and z rows follow from blockIdx by integer arithmetic (the grid is
-//     the tiled element order itself), so nothing at CTA start waits on a load;
-//   * phase 1 (thread per node) needs only the TMA data: EOS + contravariant fluxes F^1, F^2 (in place of G), F^3;
-//     the cp.async traces land meanwhile;
-//   * phase 2, no barrier inside: FACE tasks (thread per face node, direction-generic code, handed out from the last
-//     thread downwards so the warp without line tasks takes the second round) turn the trace into the lifted
-//     numerical-flux part  rf = -(1/2) sJ n.F^+ - (1/2) sJ lambda (Y^- - Y^+)  in place of the trace, and LINE tasks
-//     (thread per line, one warp per direction, D from the constant bank) contract D_d F^d in place, folding the
-//     element's own half (1/2) sJ n.F^- of the face term into the line's end values from registers -- the two kinds
-//     of task touch disjoint data;
-//   * phase 3 (thread per node): all shared-memory operands loaded up front, sum of the three directions, the rf of
-//     the up to three faces the node lies on, gravity source, fused LSRK update, coalesced streaming stores.
-// Three CTA barriers; ~45 KB of shared memory per CTA at N = 4, five CTAs per SM.  Arithmetic follows
-// cm_dg_physics.cuh.  P:L<n> = paper line.
+// Lessons built in (profiles/r1c_v5.md, profiles/r1e_v9.md): at ~20 resident warps per SM (shared memory holds five
+// elements per SM) the kernels are bound by the dependent instruction chain of each warp and by the shared-memory
+// data pipe, so no warp may idle at a barrier and nothing may wait on a chain of global loads:
+//   * the launch grid IS the tiled element order: element position, neighbour ids, wall flags and z rows follow from
+//     blockIdx by integer arithmetic, no connectivity array is read;
+//   * tendency kernel (cm7_tendency_kernel):
+//       - CTA start: lane 0 of the last warp fetches the element's own Q, packed SGS fluxes G and LSRK residual by 1-D
+//         bulk TMA (cp.async.bulk ... mbarrier::complete_tx); every thread copies the neighbour traces of one or two
+//         face nodes (6 state values + the 5 SGS values the face-normal flux needs) and the z-table rows with 8-byte
+//         cp.async;
+//       - phase 1 (thread per node) needs only the TMA data: EOS + contravariant fluxes F^1, F^3 (in place of G) and
+//         F^2 (own tiles with a padded zeta-plane stride, so that no line direction has bank conflicts); the cp.async
+//         traces land meanwhile;
+//       - phase 2, no barrier inside: FACE tasks (thread per face node, direction-generic code, handed out from the
+//         last thread downwards so the warp without line tasks takes the second round) turn the trace into the lifted
+//         numerical-flux part  rf = -(1/2) sJ n.F^+ - (1/2) sJ lambda (Y^- - Y^+)  in place of the trace, and LINE
+//         tasks (thread per line, one warp per direction, D from the constant bank) contract D_d F^d in place, folding
+//         the element's own half (1/2) sJ n.F^- of the face term into the line's end values from registers -- the two
+//         kinds of task touch disjoint data;
+//       - phase 3 (thread per node): all shared-memory operands loaded up front, sum of the three directions, the rf of
+//         the up to three faces the node lies on, gravity source, fused LSRK update, coalesced streaming stores;
+//       three CTA barriers, 45.5 KB of shared memory and 92 registers per thread at N = 4 moist: five CTAs per SM;
+//   * gradient kernel (cm9_gradient_kernel, at the end of this file): its phases are short enough that the line task
+//     can own the face terms of its two end nodes; the 2 x 6 trace values are loaded into REGISTERS at CTA start (in
+//     flight together with the TMA) and consumed in phase 2: no trace buffer at all.  cm7_gradient_kernel (trace
+//     buffer, as the tendency kernel) remains for the orders whose CTAs have fewer threads than line tasks (N <= 3).
+// Arithmetic follows cm_dg_physics.cuh.  P:L<n> = paper line.
 #pragma once
 #include "cm_dg_internal.h"
 #include "cm_dg_physics.cuh"
