@@ -6,7 +6,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIBPATH = os.path.join(_HERE, "libcm_dg.so")
+_LIBPATH = os.environ.get("CM_DG_LIB", os.path.join(_HERE, "libcm_dg.so"))   # CM_DG_LIB: a differently tuned build of the same library
 
 
 class CmDgError(RuntimeError):

@@ -38,14 +38,17 @@ def _run(cmd, log):
 
 
 def build(force=False, verbose=False):
+    """CM_DG_NVCC_EXTRA (extra nvcc flags, e.g. tuning macros) and CM_DG_LIB_OUT (output path) serve kernel experiments."""
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    if not force and not _stale(LIB):
+    extra = os.environ.get("CM_DG_NVCC_EXTRA", "").split()
+    LIB = os.environ.get("CM_DG_LIB_OUT", globals()["LIB"])
+    if not force and not extra and not _stale(LIB):
         return LIB
     os.makedirs(OBJ, exist_ok=True)
     jobs = []
     for nq in NQS:
         o = os.path.join(OBJ, "kernels_nq%d.o" % nq)
-        jobs.append(([nvcc] + NVCC_FLAGS + ["-DCM_NQ=%d" % nq, "-c", os.path.join(CSRC, "cm_dg_kernels_inst.cu"), "-o", o],
+        jobs.append(([nvcc] + NVCC_FLAGS + extra + ["-DCM_NQ=%d" % nq, "-c", os.path.join(CSRC, "cm_dg_kernels_inst.cu"), "-o", o],
                      os.path.join(OBJ, "kernels_nq%d.log" % nq)))
     o_lib = os.path.join(OBJ, "lib.o")
     jobs.append(([nvcc] + NVCC_FLAGS + ["-c", os.path.join(CSRC, "cm_dg_lib.cu"), "-o", o_lib], os.path.join(OBJ, "lib.log")))

@@ -96,7 +96,13 @@ template <int Nq, bool MOIST> struct CmCfg7 {
   static constexpr size_t GRAD_SMEM = sizeof(double) * GRAD_DOUBLES;
   static constexpr int fit(size_t smem) { return (int)(233472 / (smem + 1024)); }
   static constexpr int cap(int b, int hi) { return b < 1 ? 1 : (b > hi ? hi : b); }
-  static constexpr int MINB_T = cap(fit(TEND_SMEM), cap(640 / THREADS, 16));   // >= 100 registers per thread
+#ifndef CM_T_REGTHREADS
+#define CM_T_REGTHREADS 640
+#endif
+#ifndef CM_G_REGTHREADS
+#define CM_G_REGTHREADS 896
+#endif
+  static constexpr int MINB_T = cap(fit(TEND_SMEM), cap(CM_T_REGTHREADS / THREADS, 16));   // 640: >= 100 registers per thread
   static constexpr int MINB_G = cap(fit(GRAD_SMEM), cap(896 / THREADS, 16));   // >= 72 registers per thread
 };
 
@@ -622,7 +628,7 @@ template <int Nq, bool MOIST> struct CmCfg9 {
   static constexpr int GRAD_DOUBLES = (C7::NV + 3 * C7::NS) * C7::SLOT + 2;   // Q (then s in place), ds/dxi_d, mbarrier
   static constexpr size_t GRAD_SMEM = sizeof(double) * GRAD_DOUBLES;
   static constexpr bool OK = 3 * C7::NFP <= C7::THREADS;
-  static constexpr int MINB_G = C7::cap(C7::fit(GRAD_SMEM), C7::cap(896 / C7::THREADS, 16));
+  static constexpr int MINB_G = C7::cap(C7::fit(GRAD_SMEM), C7::cap(CM_G_REGTHREADS / C7::THREADS, 16));   // 896: >= 72 registers per thread
 };
 
 // line l of direction D -> first node and zeta index.  For Nq = 5 the eta-lines are dealt to the lanes so that each

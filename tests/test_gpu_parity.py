@@ -188,3 +188,48 @@ def test_error_reporting(P):
     bad = dict(cfg4); bad["zsfc_nodes"] = np.full_like(np.asarray(cfg4["zsfc_nodes"]), 5.0e4)
     with pytest.raises(P.CmDgError):
         P.CmDg(bad)
+
+
+def test_full_size_sampled_parity(P, oracle_mod):
+    """BASELINE config 5 at its full size (96x96x48 elements, 55.3 M nodes), in the launch configuration bench.py times:
+    cm_dg_rhs on the whole mesh, compared with the oracle on sampled element columns.  The RHS of an element depends on
+    its neighbours' state and gradients, i.e. on the 2-ring: the oracle is run on the 5x5x48-element sub-brick around a
+    sampled column (periodic closure at the sub-brick's lateral edges, which the centre column does not see) and the
+    centre column's 48 elements are compared one by one.  Plus properties that hold at any size: conservation of the
+    tendency sums and of mass / energy / water over one LSRK54 step."""
+    import torch
+    cfg, Q, dt = W.config5()
+    Ex, Ey, Ez = cfg["ne"]
+    g = P.CmDg(cfg)
+    Qd = g.to_device(Q)
+    dQd = g.rhs(Qd)
+    pos_of_lex = np.empty(g.n_elem, dtype=np.int64)
+    pos_of_lex[g.lex_of_elem] = np.arange(g.n_elem)
+    npn = g.np
+    sub_cfg, _, _ = W.config5(ne=(5, 5, Ez), N=cfg["N"], hi=(5 * 6000.0 / Ex, 5 * 6000.0 / Ey, 3000.0))
+    o = oracle_mod.Oracle(sub_cfg)
+    for cx, cy in ((0, 0), (47, 50), (95, 95), (31, 16)):
+        sx = (cx + np.arange(-2, 3)) % Ex
+        sy = (cy + np.arange(-2, 3)) % Ey
+        lex = (sx[None, None, :] + Ex * (sy[None, :, None] + Ey * np.arange(Ez)[:, None, None])).reshape(-1)
+        dQo = o.rhs(np.ascontiguousarray(Q[lex]))
+        centre = 2 + 5 * (2 + 5 * np.arange(Ez))                       # sub-brick lexicographic ids of the centre column
+        full = cx + Ex * (cy + Ey * np.arange(Ez))
+        idx = (pos_of_lex[full][:, None] * npn + np.arange(npn)[None, :]).reshape(-1)
+        got = dQd[:, torch.from_numpy(idx).to(dQd.device)].cpu().numpy().T.reshape(Ez, npn, g.nvar)
+        for v in range(g.nvar):
+            scale = np.max(np.abs(dQo[..., v]))
+            err = np.max(np.abs(got[..., v] - dQo[centre][..., v])) / scale
+            assert err <= RHS_TOL, (cx, cy, v, err)
+    # conservation of the tendency (mass-weighted sums of d rho, d rho e, d rho q vanish: periodic x/y, no-flux z)
+    s = g.diagnostics(dQd)                                            # mass / energy / water fields = sums of M * dQ_f
+    a = g.diagnostics(torch.abs(dQd))
+    for key in ("mass", "energy", "water"):
+        assert abs(s[key]) <= 1e-12 * a[key], (key, s[key], a[key])
+    d0 = g.diagnostics(Qd)
+    g.lsrk_step(Qd, dt, 1)
+    d1 = g.diagnostics(Qd)
+    assert d1["n_nonfinite"] == 0
+    for key in ("mass", "energy", "water"):
+        assert abs(d1[key] - d0[key]) <= 1e-12 * abs(d0[key]), (key, d0[key], d1[key])
+    g.close()
