@@ -6,7 +6,6 @@
 
 #define CM_MAXNQ 8
 #define CM_ZTAB_W 8   // doubles per z-table row (flat meshes): Phi, rho_r, rhoe_r, rhoq_r, E_r, q_r, 1/c_vm_r, unused
-#define CM_XPLANE(NF) ((NF) + ((NF) & 1))   // doubles per x-face plane in the XQ / XG copies (16-byte multiple: bulk-TMA source)
 #define CM_NGEO 12    // general geometry, per node: Ja[9], 1/J, z, (C_s Delta)^2
 
 // Thermodynamic constants of eq. (7)-(14) in the combinations the kernels use.
@@ -37,10 +36,6 @@ struct CmKP {
   double* Gout;          // gradient output
   double* dQ;            // residual (in/out) or rhs output
   double* Qnew;          // LSRK: updated state (ping-pong buffer)
-  const double* XQ;      // flat: x-face planes of Q, [nvar][Ne][2][CM_XPLANE(NF)] contiguous (cm_dg_lib.cu: xface_extract_kernel)
-  double* XQnew;         // flat, LSRK: x-face planes of the updated state
-  const double* XG;      // flat: x-face planes of the 5 SGS values the x-normal flux needs, [5][Ne][2][CM_XPLANE(NF)]
-  double* XGout;         // flat: gradient kernel output of the same
   const int* nbr;        // [Ne][6] neighbour in library order, <0 = wall
   const int* erow;       // flat: [Ne] first z-table row of the element (= ez*Nq)
   const int* elz;        // flat: [Ne][4] z-table rows {facing row of the -z neighbour, own first row, facing row of +z, 0}; -1 = wall

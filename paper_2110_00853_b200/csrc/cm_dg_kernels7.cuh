@@ -80,20 +80,16 @@ template <int Nq, bool MOIST> struct CmCfg7 {
   static constexpr int NFP = ((NF + 31) / 32) * 32;         // line tasks of one direction, padded to whole warps
   static constexpr int ZR = Nq + 2;                         // z-table rows: facing row below, own Nq rows, facing row above
   static constexpr int ZW = 10;                             // doubles per z row in shared memory: rows fall into disjoint banks
-  static constexpr int TAIL = (ZR - 1) * ZW + 7 + 2;        // z rows (7 values used per row), 2 mbarriers
+  static constexpr int TAIL = (ZR - 1) * ZW + 7 + 1;        // z rows (7 values used per row), mbarrier
   // stride between the trace blocks of two faces: >= rows * NF and = NF (mod 16), so that consecutive face nodes of a
   // warp that straddles two faces fall into consecutive banks
   static constexpr int fstride(int rows) { return rows * NF + ((NF - rows * NF) % 16 + 16) % 16; }
-  static constexpr int TS_G = fstride(NV);
-  // tendency: trace rows of XP = NF rounded up to even doubles, so that a row is a legal bulk-TMA destination (the x and
-  // z traces are contiguous in memory and arrive by bulk TMA; a z row holds its plane at offset 0 or 1, see cm7_tma_traces)
-  static constexpr int XP = CM_XPLANE(NF);
-  static constexpr int RS_T = XP, TS_T = NTR * RS_T;
-  // F^2 tiles (tendency): own tiles in node order; cm7_yline deals the eta-lines to the lanes so that each half-warp
-  // holds whole zeta-planes {0, 1, 4} / {2, 3}: one 2-way bank conflict per access instead of two
-  static constexpr int PS2 = NF;
-  static constexpr int SLOT2 = SLOT;
-  static constexpr int TEND_DOUBLES = (NV + 2 * NV + 1 + NV) * SLOT + NV * SLOT2 + 6 * TS_T + TAIL;   // Q, F^1 F^3 (G lands there), c, residual, F^2, traces
+  static constexpr int TS_T = fstride(NTR), TS_G = fstride(NV);
+  // F^2 tiles (tendency): node (i, j, k) at i + Nq j + PS2 k.  At Nq = 5 a zeta-plane stride of 27 puts the 15 / 10
+  // eta-lines of zeta-planes {0,1,2} / {3,4} into distinct banks (cm7_yline deals the lines to the lanes that way)
+  static constexpr int PS2 = (Nq == 5) ? NF + 2 : NF;
+  static constexpr int SLOT2 = (Nq - 1) * PS2 + NF;
+  static constexpr int TEND_DOUBLES = (NV + 2 * NV + 1 + NV) * SLOT + NV * SLOT2 + 5 * TS_T + NTR * NF + TAIL;   // Q, F^1 F^3 (G lands there), c, residual, F^2, traces
   static constexpr int GRAD_DOUBLES = (NV + 3 * NS) * SLOT + 5 * TS_G + NV * NF + TAIL;            // Q (then s in place), ds/dxi_d, traces
   static_assert(2 * NV >= NG, "the packed SGS fluxes are staged in the F^1, F^3 tiles");
   static constexpr size_t TEND_SMEM = sizeof(double) * TEND_DOUBLES;
@@ -195,9 +191,8 @@ __device__ __forceinline__ void cm7_face_node(int fn, int& f, int& m, int& d, in
 }
 
 // CTA prologue shared by both kernels: z rows and neighbour traces to shared memory by cp.async.
-//   T[f * TS + v * RS + m]: value v of the node of neighbour f that coincides with face node m of face f.
-//   ONLYY: only the eta-faces (the tendency kernel brings its x and z traces by bulk TMA, cm7_tma_traces)
-template <int Nq, int NV, int NGD, int TS, int RS, bool ONLYY, int THREADS>
+//   T[f * TS + v * NF + m]: value v of the node of neighbour f that coincides with face node m of face f
+template <int Nq, int NV, int NGD, int TS, int THREADS>
 __device__ __forceinline__ void cm7_prefetch_traces(const CmKP& p, const Cm7Pos& q, int t, double* __restrict__ T,
                                                     double* __restrict__ zt) {
   constexpr int NF = Nq * Nq, NP = NF * Nq, ZR = Nq + 2;
@@ -214,62 +209,22 @@ __device__ __forceinline__ void cm7_prefetch_traces(const CmKP& p, const Cm7Pos&
   for (int fn = t; fn < 6 * NF; fn += THREADS) {
     int f, m, d, s, nm, np_, kline;
     cm7_face_node<Nq>(fn, f, m, d, s, nm, np_, kline);
-    if (!((q.wallmask >> f) & 1) && (!ONLYY || d == 1)) {
+    if (!((q.wallmask >> f) & 1)) {
       const int nb = cm7_neighbour(p, q, d, s);
+      const size_t idp = (size_t)nb * NP + np_;
       double* dst = T + f * TS + m;
-      if (d == 0) {
-        // x traces from the contiguous x-face copies: plane (s ? 0 : 1) of the neighbour, node m
-        constexpr int XP = CM_XPLANE(NF);
-        const size_t xo = (size_t)nb * (2 * XP) + (s ? 0 : XP) + m, xs = (size_t)p.Ne * (2 * XP);
-        const double* src = p.XQ + xo;
+      const double* src = p.Q + idp;
 #pragma unroll
-        for (int v = 0; v < NV; ++v) { cm7_cp8(dst + v * RS, src); src += xs; }
-        if (NGD > 0) {
-          const double* g = p.XG + xo;
+      for (int v = 0; v < NV; ++v) { cm7_cp8(dst + v * NF, src); src += p.stride; }
+      if (NGD > 0) {
+        const double* g = p.G + idp;
 #pragma unroll
-          for (int k = 0; k < NGD; ++k) { cm7_cp8(dst + (NV + k) * RS, g); g += xs; }
-        }
-      } else {
-        const size_t idp = (size_t)nb * NP + np_;
-        const double* src = p.Q + idp;
-#pragma unroll
-        for (int v = 0; v < NV; ++v) { cm7_cp8(dst + v * RS, src); src += p.stride; }
-        if (NGD > 0) {
-          const double* g = p.G + idp;
-#pragma unroll
-          for (int k = 0; k < NGD; ++k) cm7_cp8(dst + (NV + k) * RS, g + (size_t)cm7_gidx(d, k) * p.stride);
-        }
+        for (int k = 0; k < NGD; ++k) cm7_cp8(dst + (NV + k) * NF, g + (size_t)cm7_gidx(d, k) * p.stride);
       }
     }
   }
   cm7_cp_commit();
 }
-
-// tendency: the x and z neighbour traces by bulk TMA, issued by the 32 lanes of one warp (lane w: copies w, w + 32, ...).
-// x traces come from the contiguous x-face copies XQ / XG (planes of XP doubles, 16-byte aligned); a z trace is the
-// k = 0 or k = N plane of the neighbour's own tile: NF contiguous doubles that start on an odd double when NP is odd and
-// the neighbour id is odd -- then the copy starts one double earlier and the plane sits at offset 1 of its row
-// (bit f of `zoff`).  Completion is counted on `bar`; the caller has set its expect_tx to cm7_tma_trace_bytes.
-template <int Nq, int NV, int NGD, int TS>
-__device__ __forceinline__ void cm7_tma_traces(const CmKP& p, const Cm7Pos& q, int w, double* __restrict__ T, uint64_t* bar) {
-  constexpr int NF = Nq * Nq, NP = NF * Nq, N = Nq - 1, XP = CM_XPLANE(NF), NT = NV + NGD;
-  for (int idx = w; idx < 4 * NT; idx += 32) {
-    const int fi = idx / NT, r = idx - fi * NT;
-    const int f = (fi < 2) ? fi : fi + 2, d = f >> 1, s = f & 1;
-    if ((q.wallmask >> f) & 1) continue;
-    const int nb = cm7_neighbour(p, q, d, s);
-    const double* src;
-    if (d == 0) {
-      const size_t xo = ((size_t)nb * 2 + (s ? 0 : 1)) * XP, xs = (size_t)p.Ne * (2 * XP);
-      src = (r < NV) ? p.XQ + (size_t)r * xs + xo : p.XG + (size_t)(r - NV) * xs + xo;
-    } else {
-      const size_t zo = (size_t)nb * NP + (s ? 0 : N * NF) - ((NP & 1) ? (nb & 1) : 0);
-      src = (r < NV) ? p.Q + (size_t)r * p.stride + zo : p.G + (size_t)cm7_gidx(2, r - NV) * p.stride + zo;
-    }
-    cm7_bulk_g2s(T + f * TS + r * XP, src, XP * 8, bar);
-  }
-}
-__device__ __forceinline__ int cm7_popc4(int wallmask) { return __popc((~wallmask) & 0x33); }   // open faces among -x, +x, -z, +z
 
 // ------------------------------------------------------------------------------------------------
 // tendency, phase 2a: face task.  Replaces the trace of face node fn by
@@ -279,13 +234,13 @@ __device__ __forceinline__ int cm7_popc4(int wallmask) { return __popc((~wallmas
 // ------------------------------------------------------------------------------------------------
 template <int Nq, bool MOIST, bool SGS>
 __device__ __forceinline__ void cm7_tend_face(const CmKP& p, const double* __restrict__ Qs, const double* __restrict__ cs,
-                                              double* __restrict__ T, const double* __restrict__ zt, int wallmask, int zoff, int fn) {
+                                              double* __restrict__ T, const double* __restrict__ zt, int wallmask, int fn) {
   using C = CmCfg7<Nq, MOIST>;
-  constexpr int NF = C::NF, NV = C::NV, NGD = C::NGD, SLOT = C::SLOT, TS = C::TS_T, RS = C::RS_T;
+  constexpr int NF = C::NF, NV = C::NV, NGD = C::NGD, SLOT = C::SLOT, TS = C::TS_T;
   int f, m, d, s, nm, np_, kline;
   cm7_face_node<Nq>(fn, f, m, d, s, nm, np_, kline);
   const bool wall = (wallmask >> f) & 1;
-  double* tr = T + f * TS + ((zoff >> f) & 1) + m;
+  double* tr = T + f * TS + m;
   const double sgn = s ? 1.0 : -1.0;
   const double sJ = (d == 0) ? p.cA[0] : (d == 1) ? p.cA[1] : p.cA[2];
   const double A = sgn * sJ;
@@ -300,10 +255,10 @@ __device__ __forceinline__ void cm7_tend_face(const CmKP& p, const double* __res
   if (!wall) {
     double Yp[6], gp[5];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) Yp[v] = tr[v * RS];
+    for (int v = 0; v < NV; ++v) Yp[v] = tr[v * NF];
     if (SGS)
 #pragma unroll
-      for (int k = 0; k < NGD; ++k) gp[k] = tr[(NV + k) * RS];
+      for (int k = 0; k < NGD; ++k) gp[k] = tr[(NV + k) * NF];
     cm7_site(zt + ((d < 2) ? 1 + kline : (s ? Nq + 1 : 0)) * CM_ZSM_W, st);
     cm_eos<MOIST>(p, Yp, st, P);
     const double ud = (d == 0) ? P.u : (d == 1) ? P.v : P.w;
@@ -336,26 +291,24 @@ __device__ __forceinline__ void cm7_tend_face(const CmKP& p, const double* __res
     if (f == 4) rf[4] = sJ * p.shf;                                        // prescribed upward energy flux
   }
 #pragma unroll
-  for (int v = 0; v < NV; ++v) tr[v * RS] = rf[v];
+  for (int v = 0; v < NV; ++v) tr[v * NF] = rf[v];
 }
 
-// eta-line l -> first node in an F^2 tile; false = idle lane.  Nq = 5: lanes 0..14 hold zeta-planes 0, 1, 4, lanes
-// 16..25 planes 2, 3
+// eta-line l -> first node in an F^2 tile; false = idle lane.  Nq = 5: lanes 0..14 hold zeta-planes 0..2, lanes 16..25
+// planes 3..4 (see CmCfg7::PS2)
 template <int Nq>
 __device__ __forceinline__ bool cm7_yline(int l, int& base) {
-  constexpr int NF = Nq * Nq;
+  constexpr int NF = Nq * Nq, PS2 = (Nq == 5) ? NF + 2 : NF;
   if (Nq == 5) {
-    int a, b;
-    if (l < 10) { b = l / 5; a = l - 5 * b; }
-    else if (l < 15) { b = 4; a = l - 10; }
-    else if (l >= 16 && l < 26) { b = 2 + (l - 16) / 5; a = (l - 16) % 5; }
-    else return false;
-    base = a + NF * b;
+    if (l == 15 || l >= 26) return false;
+    const int ll = (l < 15) ? l : l - 1;              // 0..24
+    const int b = ll / 5, a = ll - 5 * b;
+    base = a + PS2 * b;
     return true;
   }
   if (l >= NF) return false;
   const int b = l / Nq, a = l - b * Nq;
-  base = a + NF * b;
+  base = a + PS2 * b;
   return true;
 }
 
@@ -392,15 +345,15 @@ template <int Nq, bool MOIST, bool SGS, int MODE>
 __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>::MINB_T) cm7_tendency_kernel(const __grid_constant__ CmKP p) {
   using C = CmCfg7<Nq, MOIST>;
   constexpr int NF = C::NF, NP = C::NP, N = Nq - 1, NV = C::NV, NG = C::NG, SLOT = C::SLOT, NFP = C::NFP, THREADS = C::THREADS;
-  constexpr int TS = C::TS_T, RS = C::RS_T, NT = SGS ? C::NTR : NV;
+  constexpr int TS = C::TS_T;
   extern __shared__ __align__(128) double smem7[];
   double* Qt = smem7;                                  // [NV][SLOT]     state
   double* Ft = Qt + NV * SLOT;                         // [2][NV][SLOT]  F^1, F^3 (the packed SGS fluxes G land here)
   double* ct = Ft + 2 * NV * SLOT;                     // [SLOT]         sound speed
   double* Rt = ct + SLOT;                              // [NV][SLOT]     LSRK residual
   double* F2 = Rt + NV * SLOT;                         // [NV][SLOT2]    F^2 (zeta-plane stride PS2)
-  double* T = F2 + NV * C::SLOT2;                      // [6][NTR][RS]   neighbour traces [v][m] per face, then rf
-  double* zt = T + 6 * TS;                             // [ZR][CM_ZSM_W]
+  double* T = F2 + NV * C::SLOT2;                          // [6][TS]        neighbour traces [v][m] per face, then rf
+  double* zt = T + 5 * TS + C::NTR * NF;      // [ZR][CM_ZSM_W]
   uint64_t* mbar = reinterpret_cast<uint64_t*>(zt + (C::ZR - 1) * CM_ZSM_W + 7);
 
   const int t = threadIdx.x;
@@ -408,30 +361,21 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
   const int e = pos.e;
   const int sh = C::ODD ? (e & 1) : 0;
 
-  // z traces: plane offset in its row (odd tile size and odd neighbour id), bits 4 and 5
-  const int zoff = C::ODD ? (((cm7_neighbour(p, pos, 2, 0) & 1) << 4) | ((cm7_neighbour(p, pos, 2, 1) & 1) << 5)) : 0;
-  if (t >= THREADS - 32) {                             // the last warp issues the bulk copies
-    const int w = t - (THREADS - 32);
-    if (w == 0) {
-      cm7_mbar_init(mbar, 1);
-      cm7_mbar_init(mbar + 1, 1);
-      cm7_fence_mbar_init();
-      const long long src = (long long)e * NP - sh;
-      cm7_mbar_expect_tx(mbar, (uint32_t)((NV + (SGS ? NG : 0) + (MODE == 1 ? NV : 0)) * SLOT * sizeof(double)));
+  if (t == THREADS - 32) {                             // lane 0 of the last warp
+    cm7_mbar_init(mbar, 1);
+    cm7_fence_mbar_init();
+    const long long src = (long long)e * NP - sh;
+    cm7_mbar_expect_tx(mbar, (uint32_t)((NV + (SGS ? NG : 0) + (MODE == 1 ? NV : 0)) * SLOT * sizeof(double)));
 #pragma unroll
-      for (int v = 0; v < NV; ++v) cm7_bulk_g2s(Qt + v * SLOT, p.Q + v * p.stride + src, SLOT * 8, mbar);
-      if (SGS)
+    for (int v = 0; v < NV; ++v) cm7_bulk_g2s(Qt + v * SLOT, p.Q + v * p.stride + src, SLOT * 8, mbar);
+    if (SGS)
 #pragma unroll
-        for (int k = 0; k < NG; ++k) cm7_bulk_g2s(Ft + k * SLOT, p.G + k * p.stride + src, SLOT * 8, mbar);
-      if (MODE == 1)
+      for (int k = 0; k < NG; ++k) cm7_bulk_g2s(Ft + k * SLOT, p.G + k * p.stride + src, SLOT * 8, mbar);
+    if (MODE == 1)
 #pragma unroll
-        for (int v = 0; v < NV; ++v) cm7_bulk_g2s(Rt + v * SLOT, p.dQ + v * p.stride + src, SLOT * 8, mbar);
-      cm7_mbar_expect_tx(mbar + 1, (uint32_t)(cm7_popc4(pos.wallmask) * NT * RS * sizeof(double)));
-    }
-    __syncwarp();
-    cm7_tma_traces<Nq, NV, SGS ? C::NGD : 0, TS>(p, pos, w, T, mbar + 1);
+      for (int v = 0; v < NV; ++v) cm7_bulk_g2s(Rt + v * SLOT, p.dQ + v * p.stride + src, SLOT * 8, mbar);
   }
-  cm7_prefetch_traces<Nq, NV, SGS ? C::NGD : 0, TS, RS, true, THREADS>(p, pos, t, T, zt);
+  cm7_prefetch_traces<Nq, NV, SGS ? C::NGD : 0, TS, THREADS>(p, pos, t, T, zt);
 
   double* Qs = Qt + sh; double* Fs = Ft + sh; double* cs = ct + sh; const double* Rs = Rt + sh;
   const int n = t;
@@ -462,12 +406,11 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
 #pragma unroll
     for (int v = 0; v < NV; ++v) { Fs[v * SLOT + n] = Fa[v]; Fs[(NV + v) * SLOT + n] = Fc[v]; F2[v * C::SLOT2 + n2] = Fb[v]; }
   }
-  cm7_cp_wait_all();                                   // this thread's eta-trace copies have landed
-  __syncthreads();                                     // fluxes, sound speed and everybody's eta traces visible
-  cm7_mbar_wait(mbar + 1, 0);                          // x and z traces (bulk TMA)
+  cm7_cp_wait_all();                                   // this thread's trace copies have landed
+  __syncthreads();                                     // fluxes, sound speed and everybody's traces visible
 
   // ---- phase 2: face tasks (from the last thread downwards) and line tasks (one warp per direction); independent
-  for (int fn = THREADS - 1 - t; fn < 6 * NF; fn += THREADS) cm7_tend_face<Nq, MOIST, SGS>(p, Qs, cs, T, zt, pos.wallmask, zoff, fn);
+  for (int fn = THREADS - 1 - t; fn < 6 * NF; fn += THREADS) cm7_tend_face<Nq, MOIST, SGS>(p, Qs, cs, T, zt, pos.wallmask, fn);
   for (int lt = t; lt < 3 * NFP; lt += THREADS) {
     const int d = lt / NFP, l = lt % NFP;
     if (d == 0) { if (l < NF) cm7_tend_line<Nq, NV, SLOT, 1, 0>(p, Fs + Nq * l, pos.wallmask); }
@@ -492,10 +435,9 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
 #pragma unroll
     for (int d = 0; d < 3; ++d)
       if (c3[d] == 0 || c3[d] == N) {
-        const int f = 2 * d + (c3[d] == N ? 1 : 0);
-        const double* tr = T + f * TS + ((zoff >> f) & 1) + m3[d];
+        const double* tr = T + (2 * d + (c3[d] == N ? 1 : 0)) * TS + m3[d];
 #pragma unroll
-        for (int v = 0; v < NV; ++v) lift[v] += tr[v * RS];
+        for (int v = 0; v < NV; ++v) lift[v] += tr[v * NF];
       }
     const size_t idx = (size_t)e * NP + n;
     double* o1 = p.dQ + idx;
@@ -509,11 +451,8 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
       } else {
         // a5: dU <- A_s dU + dt RHS ; U <- U + B_s dU
         const double dnew = (MODE == 1) ? p.rka * Ro[v] + p.dt * rhs : p.dt * rhs;
-        const double ynew = Yo[v] + p.rkb * dnew;
         __stcs(o1, dnew);
-        __stcs(o2, ynew);
-        if (i_ == 0 || i_ == N)                                  // keep the contiguous x-face copy of the new state up to date
-          p.XQnew[((size_t)v * p.Ne + e) * (2 * C::XP) + (i_ == N ? C::XP : 0) + j_ + Nq * k_] = ynew;
+        __stcs(o2, Yo[v] + p.rkb * dnew);
         o2 += p.stride;
       }
       o1 += p.stride;
@@ -599,7 +538,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
 #pragma unroll
     for (int v = 0; v < NV; ++v) cm7_bulk_g2s(Qt + v * SLOT, p.Q + v * p.stride + src, SLOT * 8, mbar);
   }
-  cm7_prefetch_traces<Nq, NV, 0, TS, NF, false, THREADS>(p, pos, t, T, zt);
+  cm7_prefetch_traces<Nq, NV, 0, TS, THREADS>(p, pos, t, T, zt);
   double* ss = Qt + sh; double* dd = dt_ + sh;
   const int n = t;
   const bool node = t < NP;
@@ -672,13 +611,6 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
       o[3 * st] = m2nu * Sxy; o[4 * st] = m2nu * Sxz; o[5 * st] = m2nu * Syz;
       o[6 * st] = mDt * Gr[3][0]; o[7 * st] = mDt * Gr[3][1]; o[8 * st] = mDt * Gr[3][2];
       if (MOIST) { o[9 * st] = mDt * Gr[4][0]; o[10 * st] = mDt * Gr[4][1]; o[11 * st] = mDt * Gr[4][2]; }
-      if (i_ == 0 || i_ == N) {
-        // contiguous copy of what the x-normal flux of the neighbour's face task needs: tau_x., (J+D)_x, d_q,x
-        const size_t xs = (size_t)p.Ne * (2 * C::XP);
-        double* x = p.XGout + (size_t)e * (2 * C::XP) + (i_ == N ? C::XP : 0) + j_ + Nq * k_;
-        x[0] = m2nu * Sxx; x[xs] = m2nu * Sxy; x[2 * xs] = m2nu * Sxz; x[3 * xs] = mDt * Gr[3][0];
-        if (MOIST) x[4 * xs] = mDt * Gr[4][0];
-      }
     }
   }
 }
@@ -801,13 +733,9 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg9<Nq, MOIST>:
 #pragma unroll
     for (int s = 0; s < 2; ++s)
       if (!((pos.wallmask >> (2 * d + s)) & 1)) {
-        const int nb = cm7_neighbour(p, pos, d, s);
-        // x traces from the contiguous x-face copies (plane (s ? 0 : 1) of the neighbour, node l), y / z from the tiles
-        const double* src = (d == 0) ? p.XQ + (size_t)nb * (2 * C::XP) + (s ? 0 : C::XP) + l
-                                     : p.Q + (size_t)nb * NP + (s ? base : base + span);
-        const size_t fs = (d == 0) ? (size_t)p.Ne * (2 * C::XP) : (size_t)p.stride;
+        const double* src = p.Q + (size_t)cm7_neighbour(p, pos, d, s) * NP + (s ? base : base + span);
 #pragma unroll
-        for (int v = 0; v < NV; ++v) { Yp[s][v] = __ldg(src); src += fs; }
+        for (int v = 0; v < NV; ++v) { Yp[s][v] = __ldg(src); src += p.stride; }
         int row = pos.ez * Nq + kline;                                   // d < 2: the neighbour node is at the same height
         if (d == 2) row = s ? ((pos.ez + 1 == p.gEz) ? 0 : (pos.ez + 1) * Nq) : ((pos.ez == 0 ? p.gEz : pos.ez) * Nq - 1);
         Php[s] = __ldg(p.ztab + (size_t)row * CM_ZTAB_W);
@@ -844,7 +772,6 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg9<Nq, MOIST>:
   // ---- phase 3: physical gradient, closure, store
   if (node) {
     const size_t idx = (size_t)e * NP + n;
-    const int k_ = n / NF, j_ = (n - k_ * NF) / Nq, i_ = n - k_ * NF - j_ * Nq;
     double Gr[5][3];
 #pragma unroll
     for (int v = 0; v < NS; ++v)
@@ -869,13 +796,6 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg9<Nq, MOIST>:
       o[3 * st] = m2nu * Sxy; o[4 * st] = m2nu * Sxz; o[5 * st] = m2nu * Syz;
       o[6 * st] = mDt * Gr[3][0]; o[7 * st] = mDt * Gr[3][1]; o[8 * st] = mDt * Gr[3][2];
       if (MOIST) { o[9 * st] = mDt * Gr[4][0]; o[10 * st] = mDt * Gr[4][1]; o[11 * st] = mDt * Gr[4][2]; }
-      if (i_ == 0 || i_ == N) {
-        // contiguous copy of what the x-normal flux of the neighbour's face task needs: tau_x., (J+D)_x, d_q,x
-        const size_t xs = (size_t)p.Ne * (2 * C::XP);
-        double* x = p.XGout + (size_t)e * (2 * C::XP) + (i_ == N ? C::XP : 0) + j_ + Nq * k_;
-        x[0] = m2nu * Sxx; x[xs] = m2nu * Sxy; x[2 * xs] = m2nu * Sxz; x[3 * xs] = mDt * Gr[3][0];
-        if (MOIST) x[4 * xs] = mDt * Gr[4][0];
-      }
     }
   }
 }

@@ -243,21 +243,6 @@ __global__ void diag_kernel(const __grid_constant__ DiagArgs a, double* __restri
   }
 }
 
-// x-face planes of the state, contiguous: XQ[((v * Ne + e) * 2 + s) * XP + m] = Q[v][e][(s ? N : 0) + Nq * m], XP = CM_XPLANE(NF).  The flat
-// kernels read their -x/+x neighbour traces from these copies: in the element tile an x-face is 25 nodes 40 bytes apart
-// (one 32-byte sector per value), which made the x traces cost more than all other loads of the tendency kernel
-// together (profiles/r1f_xface.md).  The hot kernels keep the copies up to date themselves; this kernel only seeds
-// them from a caller-provided state.
-__global__ void xface_extract_kernel(int Nq, int nvar, long long Ne, long long stride, const double* __restrict__ Q,
-                                     double* __restrict__ XQ) {
-  const long long e = blockIdx.x;
-  const int NF = Nq * Nq, NP = NF * Nq, XP = CM_XPLANE(NF);
-  for (int c = threadIdx.x; c < nvar * 2 * XP; c += blockDim.x) {
-    const int v = c / (2 * XP), r = c - v * 2 * XP, s = r / XP, m = r - s * XP;
-    XQ[((size_t)v * Ne + e) * 2 * XP + r] = (m < NF) ? Q[(size_t)v * stride + e * NP + (s ? Nq - 1 : 0) + Nq * m] : 0.0;
-  }
-}
-
 }  // namespace
 
 struct cm_dg_ctx {
@@ -274,7 +259,6 @@ struct cm_dg_ctx {
   int *d_nbr = nullptr, *d_erow = nullptr, *d_elz = nullptr, *d_lex = nullptr;
   double *d_ztab = nullptr, *d_geo = nullptr, *d_ref = nullptr, *d_G = nullptr, *d_res = nullptr, *d_Q2 = nullptr;
   double *d_zsfc = nullptr, *d_xyz_user = nullptr, *d_part = nullptr, *d_stage = nullptr;
-  double *d_XQ[2] = {nullptr, nullptr}, *d_XG = nullptr;   // flat path: contiguous copies of the x-face planes of Q (ping-pong) and of the SGS fluxes
   CmKP kp;
   cm_launch_fn launch_grad = nullptr, launch_tend = nullptr;
   // profiling
@@ -291,7 +275,6 @@ void free_ctx(cm_dg_ctx* c) {
   cudaFree(c->d_nbr); cudaFree(c->d_erow); cudaFree(c->d_elz); cudaFree(c->d_lex); cudaFree(c->d_ztab); cudaFree(c->d_geo);
   cudaFree(c->d_ref); cudaFree(c->d_G); cudaFree(c->d_res); cudaFree(c->d_Q2); cudaFree(c->d_zsfc);
   cudaFree(c->d_xyz_user); cudaFree(c->d_part); cudaFree(c->d_stage);
-  cudaFree(c->d_XQ[0]); cudaFree(c->d_XQ[1]); cudaFree(c->d_XG);
   for (auto e : c->ev) cudaEventDestroy(e);
   delete c;
 }
@@ -327,30 +310,20 @@ struct Timed {
 
 bool misaligned(const void* ptr) { return (reinterpret_cast<uintptr_t>(ptr) & 15u) != 0; }
 
-int run_xface_extract(cm_dg_ctx* c, const double* Q, double* XQ) {
-  if (!XQ) return CM_DG_OK;                            // stored-metric path: no face copies
-  Timed t(c, 2);
-  xface_extract_kernel<<<(unsigned)c->Ne, 64, 0, c->st>>>(c->Nq, c->nvar, c->Ne, c->stride, Q, XQ);
-  cudaError_t err = cudaGetLastError();
-  if (err != cudaSuccess) return fail(CM_DG_ECUDA, std::string("x-face extraction launch: ") + cudaGetErrorString(err));
-  return CM_DG_OK;
-}
-
-int run_gradient(cm_dg_ctx* c, const double* Q, const double* XQ, double* Gout, int raw) {
+int run_gradient(cm_dg_ctx* c, const double* Q, double* Gout, int raw) {
   if (misaligned(Q) || misaligned(Gout)) return fail(CM_DG_EINVAL, "state arrays must be 16-byte aligned (bulk TMA source)");
   CmKP kp = c->kp;
-  kp.Q = Q; kp.XQ = XQ; kp.XGout = c->d_XG; kp.Gout = Gout; kp.mode = raw;
+  kp.Q = Q; kp.Gout = Gout; kp.mode = raw;
   Timed t(c, 0);
   cudaError_t err = c->launch_grad(kp, c->moist, c->general, c->variant, c->st);
   if (err != cudaSuccess) return fail(CM_DG_ECUDA, std::string("gradient kernel launch: ") + cudaGetErrorString(err));
   return CM_DG_OK;
 }
 
-int run_tendency(cm_dg_ctx* c, const double* Q, const double* XQ, double* dQ, double* Qnew, double* XQnew, int mode,
-                 double rka, double rkb, double dt) {
+int run_tendency(cm_dg_ctx* c, const double* Q, double* dQ, double* Qnew, int mode, double rka, double rkb, double dt) {
   if (misaligned(Q) || misaligned(dQ) || misaligned(Qnew)) return fail(CM_DG_EINVAL, "state arrays must be 16-byte aligned (bulk TMA source)");
   CmKP kp = c->kp;
-  kp.Q = Q; kp.XQ = XQ; kp.XG = c->d_XG; kp.XQnew = XQnew; kp.G = c->d_G; kp.dQ = dQ; kp.Qnew = Qnew; kp.mode = mode; kp.rka = rka; kp.rkb = rkb; kp.dt = dt;
+  kp.Q = Q; kp.G = c->d_G; kp.dQ = dQ; kp.Qnew = Qnew; kp.mode = mode; kp.rka = rka; kp.rkb = rkb; kp.dt = dt;
   Timed t(c, 1);
   cudaError_t err = c->launch_tend(kp, c->moist, c->general, c->variant, c->st);
   if (err != cudaSuccess) return fail(CM_DG_ECUDA, std::string("tendency kernel launch: ") + cudaGetErrorString(err));
@@ -599,13 +572,6 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
 
   // ---- scratch owned by the ctx
   if (p->sgs) CM_CUDA_B(cudaMalloc(&c->d_G, (size_t)c->ngrad * fbytes));
-  if (c->variant == 7) {
-    const size_t xbytes = (size_t)Ne * 2 * CM_XPLANE(Nq * Nq) * sizeof(double);   // one field of x-face planes
-    CM_CUDA_B(cudaMalloc(&c->d_XQ[0], (size_t)c->nvar * xbytes));
-    CM_CUDA_B(cudaMalloc(&c->d_XQ[1], (size_t)c->nvar * xbytes));
-    if (p->sgs) { CM_CUDA_B(cudaMalloc(&c->d_XG, (size_t)5 * xbytes)); CM_CUDA_B(cudaMemsetAsync(c->d_XG, 0, (size_t)5 * xbytes, c->st)); }
-    CM_CUDA_B(cudaMemsetAsync(c->d_XQ[1], 0, (size_t)c->nvar * xbytes, c->st));
-  }
   CM_CUDA_B(cudaMalloc(&c->d_part, (size_t)Ne * 7 * sizeof(double)));
   // residual and ping-pong state are allocated on first use by cm_dg_lsrk_step
 
@@ -653,17 +619,15 @@ int cm_dg_metrics(cm_dg_ctx* ctx, double* Ja_dev, double* J_dev) {
 
 int cm_dg_gradient(cm_dg_ctx* ctx, const double* Q_dev, double* G_dev) {
   if (!ctx || !Q_dev || !G_dev) return fail(CM_DG_EINVAL, "cm_dg_gradient: NULL argument");
-  int rc = run_xface_extract(ctx, Q_dev, ctx->d_XQ[0]); if (rc) return rc;
-  return run_gradient(ctx, Q_dev, ctx->d_XQ[0], G_dev, 1);
+  return run_gradient(ctx, Q_dev, G_dev, 1);
 }
 
 int cm_dg_rhs(cm_dg_ctx* ctx, const double* Q_dev, double* dQ_dev, double t) {
   (void)t;   // no time-dependent forcing on this path (reading R14)
   if (!ctx || !Q_dev || !dQ_dev) return fail(CM_DG_EINVAL, "cm_dg_rhs: NULL argument");
   if (Q_dev == dQ_dev) return fail(CM_DG_EINVAL, "cm_dg_rhs: Q and dQ must be distinct buffers");
-  int rc = run_xface_extract(ctx, Q_dev, ctx->d_XQ[0]); if (rc) return rc;
-  if (ctx->prm.sgs) { rc = run_gradient(ctx, Q_dev, ctx->d_XQ[0], ctx->d_G, 0); if (rc) return rc; }
-  return run_tendency(ctx, Q_dev, ctx->d_XQ[0], dQ_dev, nullptr, nullptr, 0, 0.0, 0.0, 0.0);
+  if (ctx->prm.sgs) { int rc = run_gradient(ctx, Q_dev, ctx->d_G, 0); if (rc) return rc; }
+  return run_tendency(ctx, Q_dev, dQ_dev, nullptr, 0, 0.0, 0.0, 0.0);
 }
 
 int cm_dg_lsrk_step(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t nsteps) {
@@ -674,14 +638,12 @@ int cm_dg_lsrk_step(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t 
   if (!ctx->d_res) CM_CUDA(cudaMalloc(&ctx->d_res, bytes));
   if (!ctx->d_Q2) { CM_CUDA(cudaMalloc(&ctx->d_Q2, bytes)); CM_CUDA(cudaMemsetAsync(ctx->d_Q2, 0, bytes, ctx->st)); }
   double* cur = Q_dev; double* oth = ctx->d_Q2;
-  double* xcur = ctx->d_XQ[0]; double* xoth = ctx->d_XQ[1];
-  if (nsteps > 0) { int rc = run_xface_extract(ctx, Q_dev, xcur); if (rc) return rc; }
   for (int s = 0; s < nsteps; ++s)
     for (int st = 0; st < 5; ++st) {
-      if (ctx->prm.sgs) { int rc = run_gradient(ctx, cur, xcur, ctx->d_G, 0); if (rc) return rc; }
-      int rc = run_tendency(ctx, cur, xcur, ctx->d_res, oth, xoth, 1, kRKA[st], kRKB[st], dt);
+      if (ctx->prm.sgs) { int rc = run_gradient(ctx, cur, ctx->d_G, 0); if (rc) return rc; }
+      int rc = run_tendency(ctx, cur, ctx->d_res, oth, 1, kRKA[st], kRKB[st], dt);
       if (rc) return rc;
-      std::swap(cur, oth); std::swap(xcur, xoth);
+      std::swap(cur, oth);
     }
   if (cur != Q_dev) {
     Timed tm(ctx, 2);
