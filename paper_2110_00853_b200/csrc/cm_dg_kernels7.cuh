@@ -206,7 +206,7 @@ __device__ __forceinline__ void cm7_prefetch_traces(const CmKP& p, const Cm7Pos&
   }
   cm7_cp_commit();
   // group 1: neighbour traces (phase 2 needs them)
-  for (int fn = t; fn < 6 * NF; fn += THREADS) {
+  for (int fn = THREADS - 1 - t; fn < 6 * NF; fn += THREADS) {   // the thread that will run the face task of node fn
     int f, m, d, s, nm, np_, kline;
     cm7_face_node<Nq>(fn, f, m, d, s, nm, np_, kline);
     if (!((q.wallmask >> f) & 1)) {
@@ -406,17 +406,19 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
 #pragma unroll
     for (int v = 0; v < NV; ++v) { Fs[v * SLOT + n] = Fa[v]; Fs[(NV + v) * SLOT + n] = Fc[v]; F2[v * C::SLOT2 + n2] = Fb[v]; }
   }
-  cm7_cp_wait_all();                                   // this thread's trace copies have landed
-  __syncthreads();                                     // fluxes, sound speed and everybody's traces visible
+  __syncthreads();                                     // fluxes and sound speed visible
 
-  // ---- phase 2: face tasks (from the last thread downwards) and line tasks (one warp per direction); independent
-  for (int fn = THREADS - 1 - t; fn < 6 * NF; fn += THREADS) cm7_tend_face<Nq, MOIST, SGS>(p, Qs, cs, T, zt, pos.wallmask, fn);
+  // ---- phase 2: line tasks (one warp per direction), then face tasks (from the last thread downwards: the warp
+  // without line tasks takes the second round).  Independent of each other; a face task needs only the traces its own
+  // thread has copied, so the wait for them sits behind the line task and no CTA barrier is needed for the traces
   for (int lt = t; lt < 3 * NFP; lt += THREADS) {
     const int d = lt / NFP, l = lt % NFP;
     if (d == 0) { if (l < NF) cm7_tend_line<Nq, NV, SLOT, 1, 0>(p, Fs + Nq * l, pos.wallmask); }
     else if (d == 1) { int base; if (cm7_yline<Nq>(l, base)) cm7_tend_line<Nq, NV, C::SLOT2, Nq, 1>(p, F2 + base, pos.wallmask); }
     else { if (l < NF) cm7_tend_line<Nq, NV, SLOT, NF, 2>(p, Fs + NV * SLOT + l, pos.wallmask); }
   }
+  cm7_cp_wait_all();                                   // this thread's trace copies have landed
+  for (int fn = THREADS - 1 - t; fn < 6 * NF; fn += THREADS) cm7_tend_face<Nq, MOIST, SGS>(p, Qs, cs, T, zt, pos.wallmask, fn);
   __syncthreads();
 
   // ---- phase 3: assemble the tendency of the own node and update
