@@ -56,6 +56,10 @@ __device__ __forceinline__ void cm7_bulk_g2s(void* dst, const void* src, uint32_
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(cm7_saddr(dst)),
                "l"(src), "r"(bytes), "r"(cm7_saddr(bar)) : "memory");
 }
+// L2 prefetch of a contiguous range (16-byte aligned address and size): no destination, no completion to wait for
+__device__ __forceinline__ void cm7_prefetch_l2(const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void cm7_fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void cm7_cp8(void* dst, const void* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(cm7_saddr(dst)), "l"(src) : "memory");
@@ -374,6 +378,18 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
     if (MODE == 1)
 #pragma unroll
       for (int v = 0; v < NV; ++v) cm7_bulk_g2s(Rt + v * SLOT, p.dQ + v * p.stride + src, SLOT * 8, mbar);
+  } else if (t > THREADS - 32 && p.ahead > 0 && e + p.ahead < p.Ne) {
+    // the other lanes of that warp pull the tiles of the element `ahead` places further on in the launch order into L2:
+    // its own bulk copies and the trace gathers of its neighbours then hit L2 instead of waiting on DRAM
+    constexpr int NTILE = NV + (SGS ? NG : 0) + (MODE == 1 ? NV : 0);
+    const int ea = e + p.ahead;
+    const long long src = (long long)ea * NP - (C::ODD ? (ea & 1) : 0);
+    for (int j = t - (THREADS - 32) - 1; j < NTILE; j += 31) {
+      const bool isq = j < NV, isg = SGS && !isq && j < NV + NG;
+      const int idx = isq ? j : isg ? j - NV : j - NV - (SGS ? NG : 0);
+      const double* g = isq ? p.Q : isg ? p.G : p.dQ;
+      cm7_prefetch_l2(g + (size_t)idx * p.stride + src, SLOT * 8);
+    }
   }
   cm7_prefetch_traces<Nq, NV, SGS ? C::NGD : 0, TS, THREADS>(p, pos, t, T, zt);
 
@@ -714,6 +730,10 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg9<Nq, MOIST>:
     cm7_mbar_expect_tx(mbar, (uint32_t)(NV * SLOT * sizeof(double)));
 #pragma unroll
     for (int v = 0; v < NV; ++v) cm7_bulk_g2s(Qt + v * SLOT, p.Q + v * p.stride + src, SLOT * 8, mbar);
+  } else if (t > THREADS - 32 && t <= THREADS - 32 + NV && p.ahead > 0 && e + p.ahead < p.Ne) {
+    // L2 prefetch of the state tiles of the element `ahead` places further on in the launch order (see the tendency kernel)
+    const int ea = e + p.ahead, v = t - (THREADS - 32) - 1;
+    cm7_prefetch_l2(p.Q + (size_t)v * p.stride + ((long long)ea * NP - (C::ODD ? (ea & 1) : 0)), SLOT * 8);
   }
 
   // ---- the thread's line task and the neighbour traces of its two end nodes, into registers

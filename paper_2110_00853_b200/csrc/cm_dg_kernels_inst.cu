@@ -59,6 +59,15 @@ cudaError_t launch_tend2(const CmKP& kp, cudaStream_t st) {
 }
 
 
+// one wave of resident CTAs = the L2 prefetch distance of the flat kernels (CmKP::ahead < 0)
+template <typename K>
+int wave_size(K kernel, int threads, size_t smem) {
+  int dev = 0, sms = 0, per_sm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess) return 0;
+  return sms * per_sm;
+}
+
 template <int Nq, bool MOIST, bool RAW>
 cudaError_t launch_grad7(const CmKP& kp, cudaStream_t st) {
   using C = CmCfg7<Nq, MOIST>;
@@ -67,9 +76,14 @@ cudaError_t launch_grad7(const CmKP& kp, cudaStream_t st) {
   if constexpr (CmCfg9<Nq, MOIST>::OK) {
     // every line task has its own thread: register-staged traces (cm9_gradient_kernel)
     constexpr size_t smem = CmCfg9<Nq, MOIST>::GRAD_SMEM;
+    static int wave = 0;
+    const bool first = !configured;
     cudaError_t err = configure(cm9_gradient_kernel<Nq, MOIST, RAW>, smem, configured);
     if (err != cudaSuccess) return err;
-    cm9_gradient_kernel<Nq, MOIST, RAW><<<grid, C::THREADS, smem, st>>>(kp);
+    if (first) wave = wave_size(cm9_gradient_kernel<Nq, MOIST, RAW>, C::THREADS, smem);
+    CmKP k2 = kp;
+    if (k2.ahead < 0) k2.ahead = wave;
+    cm9_gradient_kernel<Nq, MOIST, RAW><<<grid, C::THREADS, smem, st>>>(k2);
   } else {
     cudaError_t err = configure(cm7_gradient_kernel<Nq, MOIST, RAW>, C::GRAD_SMEM, configured);
     if (err != cudaSuccess) return err;
@@ -82,9 +96,14 @@ template <int Nq, bool MOIST, bool SGS, int MODE>
 cudaError_t launch_tend7(const CmKP& kp, cudaStream_t st) {
   using C = CmCfg7<Nq, MOIST>;
   static bool configured = false;
+  static int wave = 0;
+  const bool first = !configured;
   cudaError_t err = configure(cm7_tendency_kernel<Nq, MOIST, SGS, MODE>, C::TEND_SMEM, configured);
   if (err != cudaSuccess) return err;
-  cm7_tendency_kernel<Nq, MOIST, SGS, MODE><<<dim3(kp.gPY * kp.gL, kp.gEz, kp.gNXC * kp.gNYP), C::THREADS, C::TEND_SMEM, st>>>(kp);
+  if (first) wave = wave_size(cm7_tendency_kernel<Nq, MOIST, SGS, MODE>, C::THREADS, C::TEND_SMEM);
+  CmKP k2 = kp;
+  if (k2.ahead < 0) k2.ahead = wave;
+  cm7_tendency_kernel<Nq, MOIST, SGS, MODE><<<dim3(kp.gPY * kp.gL, kp.gEz, kp.gNXC * kp.gNYP), C::THREADS, C::TEND_SMEM, st>>>(k2);
   return cudaGetLastError();
 }
 

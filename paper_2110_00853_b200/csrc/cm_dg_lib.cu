@@ -261,6 +261,7 @@ struct cm_dg_ctx {
   double *d_zsfc = nullptr, *d_xyz_user = nullptr, *d_part = nullptr, *d_stage = nullptr;
   CmKP kp;
   cm_launch_fn launch_grad = nullptr, launch_tend = nullptr;
+  int ahead_t = -1, ahead_g = -1;   // L2 prefetch distance of the tendency / gradient kernel (-1 = one wave)
   // profiling
   bool profiling = false;
   std::vector<cudaEvent_t> ev;   // pairs (start, stop)
@@ -313,7 +314,7 @@ bool misaligned(const void* ptr) { return (reinterpret_cast<uintptr_t>(ptr) & 15
 int run_gradient(cm_dg_ctx* c, const double* Q, double* Gout, int raw) {
   if (misaligned(Q) || misaligned(Gout)) return fail(CM_DG_EINVAL, "state arrays must be 16-byte aligned (bulk TMA source)");
   CmKP kp = c->kp;
-  kp.Q = Q; kp.Gout = Gout; kp.mode = raw;
+  kp.Q = Q; kp.Gout = Gout; kp.mode = raw; kp.ahead = c->ahead_g;
   Timed t(c, 0);
   cudaError_t err = c->launch_grad(kp, c->moist, c->general, c->variant, c->st);
   if (err != cudaSuccess) return fail(CM_DG_ECUDA, std::string("gradient kernel launch: ") + cudaGetErrorString(err));
@@ -323,6 +324,7 @@ int run_gradient(cm_dg_ctx* c, const double* Q, double* Gout, int raw) {
 int run_tendency(cm_dg_ctx* c, const double* Q, double* dQ, double* Qnew, int mode, double rka, double rkb, double dt) {
   if (misaligned(Q) || misaligned(dQ) || misaligned(Qnew)) return fail(CM_DG_EINVAL, "state arrays must be 16-byte aligned (bulk TMA source)");
   CmKP kp = c->kp;
+  kp.ahead = c->ahead_t;
   kp.Q = Q; kp.G = c->d_G; kp.dQ = dQ; kp.Qnew = Qnew; kp.mode = mode; kp.rka = rka; kp.rkb = rkb; kp.dt = dt;
   Timed t(c, 1);
   cudaError_t err = c->launch_tend(kp, c->moist, c->general, c->variant, c->st);
@@ -488,6 +490,9 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   kp.ginvL = 1.0f / (float)L; kp.ginvNXC = 1.0f / (float)(p->ne[0] / L);
   kp.gL = L; kp.gPY = PY; kp.gNXC = p->ne[0] / L; kp.gNYP = p->ne[1] / PY; kp.gEz = p->ne[2];
   for (int d = 0; d < 3; ++d) kp.gbc[d] = p->bc[d];
+  kp.ahead = -1;   // L2 prefetch distance: -1 = one wave of resident CTAs (set by the launcher); CM_DG_AHEAD_T / _G override
+  if (const char* ah = std::getenv("CM_DG_AHEAD_T")) c->ahead_t = std::atoi(ah);
+  if (const char* ah = std::getenv("CM_DG_AHEAD_G")) c->ahead_g = std::atoi(ah);
   if ((int64_t)PY * L > 2147483647LL || p->ne[2] > 65535 || (int64_t)kp.gNXC * kp.gNYP > 65535) {
     fail(CM_DG_EINVAL, "cm_dg_setup: mesh exceeds the launch-grid limits (Ez and (Ex/L)*(Ey/PY) must be <= 65535)");
     return bail(CM_DG_EINVAL);
