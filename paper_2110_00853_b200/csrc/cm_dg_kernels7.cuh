@@ -60,6 +60,11 @@ __device__ __forceinline__ void cm7_bulk_g2s(void* dst, const void* src, uint32_
 __device__ __forceinline__ void cm7_prefetch_l2(const void* src, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
+// same with the shared-memory addresses already converted (issue loops: one add per operand and copy)
+__device__ __forceinline__ void cm7_bulk_g2s_raw(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+               "r"(bytes), "r"(bar) : "memory");
+}
 __device__ __forceinline__ void cm7_fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void cm7_cp8(void* dst, const void* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(cm7_saddr(dst)), "l"(src) : "memory");
@@ -365,19 +370,28 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
   const int e = pos.e;
   const int sh = C::ODD ? (e & 1) : 0;
 
-  if (t == THREADS - 32) {                             // lane 0 of the last warp
-    cm7_mbar_init(mbar, 1);
-    cm7_fence_mbar_init();
+  if (t == THREADS - 32) { cm7_mbar_init(mbar, 1); cm7_fence_mbar_init(); }
+  __syncthreads();                                     // mbarrier initialised: from here on nobody waits for an instruction
+                                                       // stream of another warp, only for data
+  if (t == THREADS - 32) {                             // lane 0 of the last warp issues the bulk copies
     const long long src = (long long)e * NP - sh;
+    const uint32_t mb = cm7_saddr(mbar);
     cm7_mbar_expect_tx(mbar, (uint32_t)((NV + (SGS ? NG : 0) + (MODE == 1 ? NV : 0)) * SLOT * sizeof(double)));
+    {
+      const double* g = p.Q + src; uint32_t d = cm7_saddr(Qt);
 #pragma unroll
-    for (int v = 0; v < NV; ++v) cm7_bulk_g2s(Qt + v * SLOT, p.Q + v * p.stride + src, SLOT * 8, mbar);
-    if (SGS)
+      for (int v = 0; v < NV; ++v) { cm7_bulk_g2s_raw(d, g, SLOT * 8, mb); g += p.stride; d += SLOT * 8; }
+    }
+    if (SGS) {
+      const double* g = p.G + src; uint32_t d = cm7_saddr(Ft);
 #pragma unroll
-      for (int k = 0; k < NG; ++k) cm7_bulk_g2s(Ft + k * SLOT, p.G + k * p.stride + src, SLOT * 8, mbar);
-    if (MODE == 1)
+      for (int k = 0; k < NG; ++k) { cm7_bulk_g2s_raw(d, g, SLOT * 8, mb); g += p.stride; d += SLOT * 8; }
+    }
+    if (MODE == 1) {
+      const double* g = p.dQ + src; uint32_t d = cm7_saddr(Rt);
 #pragma unroll
-      for (int v = 0; v < NV; ++v) cm7_bulk_g2s(Rt + v * SLOT, p.dQ + v * p.stride + src, SLOT * 8, mbar);
+      for (int v = 0; v < NV; ++v) { cm7_bulk_g2s_raw(d, g, SLOT * 8, mb); g += p.stride; d += SLOT * 8; }
+    }
   } else if (t > THREADS - 32 && p.ahead > 0 && e + p.ahead < p.Ne) {
     // the other lanes of that warp pull the tiles of the element `ahead` places further on in the launch order into L2:
     // its own bulk copies and the trace gathers of its neighbours then hit L2 instead of waiting on DRAM
@@ -398,15 +412,18 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
   const bool node = t < NP;
   const int k_ = n / NF, j_ = (n - k_ * NF) / Nq, i_ = n - k_ * NF - j_ * Nq;
   const int n2 = n + (C::PS2 - NF) * k_;               // index in the F^2 tiles
-  cm7_cp_wait_but_one();                               // this thread's z-row copies have landed
-  __syncthreads();                                     // mbarrier init and z rows visible
+  CmSite st;                                           // own row of the z table through the read-only path (L1-resident): the
+  if (node) {                                          // shared-memory copy of the z rows is only needed by the face tasks
+    const double2* zr = reinterpret_cast<const double2*>(p.ztab + (size_t)(pos.ez * Nq + k_) * CM_ZTAB_W);
+    const double2 a = __ldg(zr), b = __ldg(zr + 1), c = __ldg(zr + 2), d = __ldg(zr + 3);
+    st.Phi = a.x; st.rho_r = a.y; st.rhoe_r = b.x; st.rhoq_r = b.y; st.E_r = c.x; st.q_r = c.y; st.icvm_r = d.x;
+  }
   cm7_mbar_wait(mbar, 0);
 
   // ---- phase 1: primitives and contravariant fluxes of the own node (F^1, F^2 overwrite G in place)
   double buoy = 0.0;
   if (node) {
-    double Y[6], g[12]; CmPrim P; CmSite st;
-    cm7_site(zt + (1 + k_) * CM_ZSM_W, st);
+    double Y[6], g[12]; CmPrim P;
 #pragma unroll
     for (int v = 0; v < NV; ++v) Y[v] = Qs[v * SLOT + n];
     if (SGS)
@@ -422,7 +439,8 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
 #pragma unroll
     for (int v = 0; v < NV; ++v) { Fs[v * SLOT + n] = Fa[v]; Fs[(NV + v) * SLOT + n] = Fc[v]; F2[v * C::SLOT2 + n2] = Fb[v]; }
   }
-  __syncthreads();                                     // fluxes and sound speed visible
+  cm7_cp_wait_but_one();                               // this thread's z-row copies have landed
+  __syncthreads();                                     // fluxes, sound speed and z rows visible
 
   // ---- phase 2: line tasks (one warp per direction), then face tasks (from the last thread downwards: the warp
   // without line tasks takes the second round).  Independent of each other; a face task needs only the traces its own
