@@ -1,7 +1,7 @@
 // cm_dg_kernels7.cuh -- the hot kernels for flat bricks (GEOM == 0): one small CTA per element, every input staged
 // asynchronously at CTA start, face work and line work decoupled so that all warps stay busy.
 //
-// Lessons built in (profiles/r1c_v5.md, profiles/r1e_v9.md): at ~20 resident warps per SM (shared memory holds five
+// Lessons built in (profiles/r1c_v5.md, profiles/r1e_v9.md, profiles/r1f_prefetch.md): at ~20 resident warps per SM (shared memory holds five
 // elements per SM) the kernels are bound by the dependent instruction chain of each warp and by the shared-memory
 // data pipe, so no warp may idle at a barrier and nothing may wait on a chain of global loads:
 //   * the launch grid IS the tiled element order: element position, neighbour ids, wall flags and z rows follow from
@@ -23,6 +23,9 @@
 //       - phase 3 (thread per node): all shared-memory operands loaded up front, sum of the three directions, the rf of
 //         the up to three faces the node lies on, gravity source, fused LSRK update, coalesced streaming stores;
 //       three CTA barriers, 45.5 KB of shared memory and 92 registers per thread at N = 4 moist: five CTAs per SM;
+//   * both kernels: the lanes next to the one that issues the bulk copies prefetch the tiles of the element one wave of
+//     resident CTAs further on in the launch order into L2 (cp.async.bulk.prefetch.L2), so that bulk copies and trace
+//     gathers hit L2 instead of waiting on DRAM (CmKP::ahead);
 //   * gradient kernel (cm9_gradient_kernel, at the end of this file): its phases are short enough that the line task
 //     can own the face terms of its two end nodes; the 2 x 6 trace values are loaded into REGISTERS at CTA start (in
 //     flight together with the TMA) and consumed in phase 2: no trace buffer at all.  cm7_gradient_kernel (trace
@@ -422,8 +425,9 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
 
   // ---- phase 1: primitives and contravariant fluxes of the own node (F^1, F^2 overwrite G in place)
   double buoy = 0.0;
+  double Y[6];                                         // the node's state stays in registers until the update in phase 3
   if (node) {
-    double Y[6], g[12]; CmPrim P;
+    double g[12]; CmPrim P;
 #pragma unroll
     for (int v = 0; v < NV; ++v) Y[v] = Qs[v * SLOT + n];
     if (SGS)
@@ -462,7 +466,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
     for (int v = 0; v < NV; ++v) {
       acc[v] = Fs[v * SLOT + n] + F2[v * C::SLOT2 + n2] + Fs[(NV + v) * SLOT + n];
       lift[v] = 0.0;
-      if (MODE != 0) Yo[v] = Qs[v * SLOT + n];
+      if (MODE != 0) Yo[v] = Y[v];
       if (MODE == 1) Ro[v] = Rs[v * SLOT + n];
     }
     // rf of the faces the node lies on
@@ -573,6 +577,9 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
     cm7_mbar_expect_tx(mbar, (uint32_t)(NV * SLOT * sizeof(double)));
 #pragma unroll
     for (int v = 0; v < NV; ++v) cm7_bulk_g2s(Qt + v * SLOT, p.Q + v * p.stride + src, SLOT * 8, mbar);
+  } else if (t > THREADS - 32 && t <= THREADS - 32 + NV && p.ahead > 0 && e + p.ahead < p.Ne) {
+    const int ea = e + p.ahead, v = t - (THREADS - 32) - 1;   // L2 prefetch one wave ahead (see the tendency kernel)
+    cm7_prefetch_l2(p.Q + (size_t)v * p.stride + ((long long)ea * NP - (C::ODD ? (ea & 1) : 0)), SLOT * 8);
   }
   cm7_prefetch_traces<Nq, NV, 0, TS, THREADS>(p, pos, t, T, zt);
   double* ss = Qt + sh; double* dd = dt_ + sh;
@@ -656,7 +663,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
 // terms of its two end nodes.  Its 2 x NV neighbour-trace values are loaded into REGISTERS at CTA start (the addresses
 // follow from blockIdx, so the loads are in flight together with the bulk TMA of the element's own tiles) and are
 // consumed only in phase 2: no trace buffer, no cp.async, no second pass over the face nodes, and the lifted jumps
-// are folded into the line's end values -- half the shared-memory traffic of cm7_gradient_kernel (profiles/r1d_v7.md:
+// are folded into the line's end values -- half the shared-memory traffic of cm7_gradient_kernel (profiles/r1e_v9.md:
 // that kernel kept the shared-memory data pipe 78 % busy).
 // ------------------------------------------------------------------------------------------------
 template <int Nq, bool MOIST> struct CmCfg9 {

@@ -85,9 +85,14 @@ cudaError_t launch_grad7(const CmKP& kp, cudaStream_t st) {
     if (k2.ahead < 0) k2.ahead = wave;
     cm9_gradient_kernel<Nq, MOIST, RAW><<<grid, C::THREADS, smem, st>>>(k2);
   } else {
+    static int wave = 0;
+    const bool first = !configured;
     cudaError_t err = configure(cm7_gradient_kernel<Nq, MOIST, RAW>, C::GRAD_SMEM, configured);
     if (err != cudaSuccess) return err;
-    cm7_gradient_kernel<Nq, MOIST, RAW><<<grid, C::THREADS, C::GRAD_SMEM, st>>>(kp);
+    if (first) wave = wave_size(cm7_gradient_kernel<Nq, MOIST, RAW>, C::THREADS, C::GRAD_SMEM);
+    CmKP k2 = kp;
+    if (k2.ahead < 0) k2.ahead = wave;
+    cm7_gradient_kernel<Nq, MOIST, RAW><<<grid, C::THREADS, C::GRAD_SMEM, st>>>(k2);
   }
   return cudaGetLastError();
 }

@@ -79,11 +79,13 @@ def test_rhs_parity_general_path_on_flat_mesh(P, oracle_mod, monkeypatch):
 
 
 @pytest.mark.parametrize("env", [{"CM_DG_SEGLEN": "1"}, {"CM_DG_SEGLEN": "2", "CM_DG_PATCH": "2"}, {"CM_DG_SEGLEN": "3", "CM_DG_PATCH": "3"},
-                                 {"CM_DG_KERNEL": "2"}])
+                                 {"CM_DG_KERNEL": "2"}, {"CM_DG_AHEAD_T": "1", "CM_DG_AHEAD_G": "2"},
+                                 {"CM_DG_AHEAD_T": "0", "CM_DG_AHEAD_G": "0"}])
 @pytest.mark.parametrize("k", [1, 3, 5])
 def test_parity_schedule_variants(P, oracle_mod, monkeypatch, env, k):
-    """Segment length / patch width of the x-sweep kernels (segment ends take the global-trace path, interiors the
-    shared-memory path) and the thread-per-node kernels on flat meshes: RHS and 7 fused steps against the oracle."""
+    """Tile shape of the element order (x-chunk length / y-patch height, i.e. the launch grid of the flat kernels), the
+    thread-per-node kernels on flat meshes, and the L2 prefetch distance (small meshes are shorter than one wave, so the
+    default distance never prefetches there): RHS and 7 fused steps against the oracle."""
     for key, val in env.items():
         monkeypatch.setenv(key, val)
     cfg, Q, dt = small_config(k)
