@@ -37,9 +37,8 @@ struct CmKP {
   double* Gout;          // gradient output
   double* dQ;            // residual (in/out) or rhs output
   double* Qnew;          // LSRK: updated state (ping-pong buffer)
-  const int* nbr;        // [Ne][6] neighbour in library order, <0 = wall
+  const int* nbr;        // [Ne][6] neighbour in library order, <0 = wall (stored-metric kernels; the flat ones compute it)
   const int* erow;       // flat: [Ne] first z-table row of the element (= ez*Nq)
-  const int* elz;        // flat: [Ne][4] z-table rows {facing row of the -z neighbour, own first row, facing row of +z, 0}; -1 = wall
   const double* ztab;    // flat: [Ez*Nq][CM_ZTAB_W]
   const double* geo;     // general: [CM_NGEO][stride]
   const double* ref;     // general: [3][stride] rho_r, rhoe_r, rhoq_r

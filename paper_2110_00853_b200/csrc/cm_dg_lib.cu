@@ -256,7 +256,7 @@ struct cm_dg_ctx {
   double xi[CM_MAXNQ], w[CM_MAXNQ], D[CM_MAXNQ][CM_MAXNQ];
   double h[3], min_node_dx;
   // device
-  int *d_nbr = nullptr, *d_erow = nullptr, *d_elz = nullptr, *d_lex = nullptr;
+  int *d_nbr = nullptr, *d_erow = nullptr, *d_lex = nullptr;
   double *d_ztab = nullptr, *d_geo = nullptr, *d_ref = nullptr, *d_G = nullptr, *d_res = nullptr, *d_Q2 = nullptr;
   double *d_zsfc = nullptr, *d_xyz_user = nullptr, *d_part = nullptr, *d_stage = nullptr;
   CmKP kp;
@@ -273,7 +273,7 @@ namespace {
 
 void free_ctx(cm_dg_ctx* c) {
   if (!c) return;
-  cudaFree(c->d_nbr); cudaFree(c->d_erow); cudaFree(c->d_elz); cudaFree(c->d_lex); cudaFree(c->d_ztab); cudaFree(c->d_geo);
+  cudaFree(c->d_nbr); cudaFree(c->d_erow); cudaFree(c->d_lex); cudaFree(c->d_ztab); cudaFree(c->d_geo);
   cudaFree(c->d_ref); cudaFree(c->d_G); cudaFree(c->d_res); cudaFree(c->d_Q2); cudaFree(c->d_zsfc);
   cudaFree(c->d_xyz_user); cudaFree(c->d_part); cudaFree(c->d_stage);
   for (auto e : c->ev) cudaEventDestroy(e);
@@ -456,17 +456,6 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   CM_CUDA_B(cudaMalloc(&c->d_nbr, nbr.size() * sizeof(int32_t)));
   CM_CUDA_B(cudaMalloc(&c->d_erow, erow.size() * sizeof(int32_t)));
   CM_CUDA_B(cudaMalloc(&c->d_lex, (size_t)Ne * sizeof(int32_t)));
-  {
-    std::vector<int32_t> elz((size_t)Ne * 4, 0);
-    for (int64_t e = 0; e < Ne; ++e) {
-      const int32_t lo_nb = nbr[e * 6 + 4], hi_nb = nbr[e * 6 + 5];
-      elz[e * 4 + 0] = (lo_nb >= 0) ? erow[lo_nb] + Nq - 1 : -1;
-      elz[e * 4 + 1] = erow[e];
-      elz[e * 4 + 2] = (hi_nb >= 0) ? erow[hi_nb] : -1;
-    }
-    CM_CUDA_B(cudaMalloc(&c->d_elz, elz.size() * sizeof(int32_t)));
-    CM_CUDA_B(cudaMemcpy(c->d_elz, elz.data(), elz.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
-  }
   CM_CUDA_B(cudaMemcpy(c->d_nbr, nbr.data(), nbr.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
   CM_CUDA_B(cudaMemcpy(c->d_erow, erow.data(), erow.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
   CM_CUDA_B(cudaMemcpy(c->d_lex, c->lex_of_elem.data(), (size_t)Ne * sizeof(int32_t), cudaMemcpyHostToDevice));
@@ -512,7 +501,7 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   kp.shf = p->shf_bottom;
   kp.inv_w0 = 1.0 / c->w[0];
   for (int i = 0; i < CM_MAXNQ; ++i) for (int j = 0; j < CM_MAXNQ; ++j) kp.D[i][j] = c->D[i][j];
-  kp.nbr = c->d_nbr; kp.erow = c->d_erow; kp.elz = c->d_elz;
+  kp.nbr = c->d_nbr; kp.erow = c->d_erow;
 
   c->min_node_dx = std::min(c->h[0], std::min(c->h[1], c->h[2])) * 0.5 * (c->xi[1] - c->xi[0]);
 
