@@ -85,7 +85,7 @@ typedef struct {
 
 /* a0: mesh, LGL nodes/weights, derivative matrix, metric terms (eq. 24), connectivity,
  * reference state.  `cuda_stream` is a cudaStream_t (NULL = default stream).  On success *out owns all
- * device scratch (geometry, gradient array, LSRK residual, second state buffer). */
+ * device scratch (geometry, gradient array, LSRK residual, two more state buffers). */
 int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out);
 
 /* Layout of state arrays: n_elem, np, field_stride (doubles) and, if non-NULL, lex_of_elem (HOST, n_elem
@@ -108,8 +108,8 @@ int cm_dg_gradient(cm_dg_ctx* ctx, const double* Q_dev, double* G_dev);
 int cm_dg_rhs(cm_dg_ctx* ctx, const double* Q_dev, double* dQ_dev, double t);
 
 /* a1-a5: advance Q by nsteps LSRK54 steps of size dt; every stage is one gradient kernel plus one fused
- * tendency + low-storage update kernel.  The result is left in Q_dev (if 5*nsteps is odd one device copy
- * from the internal ping-pong buffer is appended). */
+ * tendency + low-storage update kernel.  The result is left in Q_dev: the five stages of a step cycle through two
+ * ctx-owned buffers and end in the caller's array (no stage updates in place, no copy is appended). */
 int cm_dg_lsrk_step(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t nsteps);
 
 /* a6: conservation integrals etc. of Q_dev into *out_host; synchronises the stream. */

@@ -257,7 +257,7 @@ struct cm_dg_ctx {
   double h[3], min_node_dx;
   // device
   int *d_nbr = nullptr, *d_erow = nullptr, *d_lex = nullptr;
-  double *d_ztab = nullptr, *d_geo = nullptr, *d_ref = nullptr, *d_G = nullptr, *d_res = nullptr, *d_Q2 = nullptr;
+  double *d_ztab = nullptr, *d_geo = nullptr, *d_ref = nullptr, *d_G = nullptr, *d_res = nullptr, *d_Q2 = nullptr, *d_Q3 = nullptr;
   double *d_zsfc = nullptr, *d_xyz_user = nullptr, *d_part = nullptr, *d_stage = nullptr;
   CmKP kp;
   cm_launch_fn launch_grad = nullptr, launch_tend = nullptr;
@@ -274,7 +274,7 @@ namespace {
 void free_ctx(cm_dg_ctx* c) {
   if (!c) return;
   cudaFree(c->d_nbr); cudaFree(c->d_erow); cudaFree(c->d_lex); cudaFree(c->d_ztab); cudaFree(c->d_geo);
-  cudaFree(c->d_ref); cudaFree(c->d_G); cudaFree(c->d_res); cudaFree(c->d_Q2); cudaFree(c->d_zsfc);
+  cudaFree(c->d_ref); cudaFree(c->d_G); cudaFree(c->d_res); cudaFree(c->d_Q2); cudaFree(c->d_Q3); cudaFree(c->d_zsfc);
   cudaFree(c->d_xyz_user); cudaFree(c->d_part); cudaFree(c->d_stage);
   for (auto e : c->ev) cudaEventDestroy(e);
   delete c;
@@ -631,18 +631,16 @@ int cm_dg_lsrk_step(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t 
   const size_t bytes = (size_t)ctx->nvar * ctx->stride * sizeof(double);
   if (!ctx->d_res) CM_CUDA(cudaMalloc(&ctx->d_res, bytes));
   if (!ctx->d_Q2) { CM_CUDA(cudaMalloc(&ctx->d_Q2, bytes)); CM_CUDA(cudaMemsetAsync(ctx->d_Q2, 0, bytes, ctx->st)); }
-  double* cur = Q_dev; double* oth = ctx->d_Q2;
+  if (!ctx->d_Q3) { CM_CUDA(cudaMalloc(&ctx->d_Q3, bytes)); CM_CUDA(cudaMemsetAsync(ctx->d_Q3, 0, bytes, ctx->st)); }
+  // A stage never updates in place (neighbours still read the old state).  Three buffers in the cycle
+  // Q_dev -> Q2 -> Q3 -> Q2 -> Q3 -> Q_dev bring every step's five stages back into the caller's array: no copy.
+  double* const ring[6] = {Q_dev, ctx->d_Q2, ctx->d_Q3, ctx->d_Q2, ctx->d_Q3, Q_dev};
   for (int s = 0; s < nsteps; ++s)
     for (int st = 0; st < 5; ++st) {
-      if (ctx->prm.sgs) { int rc = run_gradient(ctx, cur, ctx->d_G, 0); if (rc) return rc; }
-      int rc = run_tendency(ctx, cur, ctx->d_res, oth, 1, kRKA[st], kRKB[st], dt);
+      if (ctx->prm.sgs) { int rc = run_gradient(ctx, ring[st], ctx->d_G, 0); if (rc) return rc; }
+      int rc = run_tendency(ctx, ring[st], ctx->d_res, ring[st + 1], 1, kRKA[st], kRKB[st], dt);
       if (rc) return rc;
-      std::swap(cur, oth);
     }
-  if (cur != Q_dev) {
-    Timed tm(ctx, 2);
-    CM_CUDA(cudaMemcpyAsync(Q_dev, cur, bytes, cudaMemcpyDeviceToDevice, ctx->st));
-  }
   return CM_DG_OK;
 }
 
