@@ -1,17 +1,15 @@
-// cm_dg_kernels2.cuh -- thread-per-node variants of the two hot kernels (the default path).
-//
-// Why a second decomposition: the column-per-thread kernels of cm_dg_kernels.cuh hold a whole column of
-// accumulators per thread (200+ registers, 90 KB shared memory per CTA) and run at 8 warps per SM; ncu shows
-// them stalled on `long_scoreboard` with the fp64 pipe 12-20 % busy (profiles/r1_first_profile.md).  Here
-//   * one thread owns ONE node, so a CTA of EPB elements x TPE threads needs ~64-100 registers per thread and
-//     several CTAs fit per SM (24+ warps): latency is hidden by thread-level parallelism;
+// cm_dg_kernels2.cuh -- thread-per-node kernels for ANY geometry (stored metric terms, per-node reference state): the
+// path of warped meshes (geom != 0) and of reference states that are not columns; on flat bricks the CTA-per-element
+// kernels of cm_dg_kernels7.cuh are used instead (CM_DG_KERNEL=2 forces these).
+//   * one thread owns ONE node, a CTA holds EPB elements x TPE threads (~64-100 registers per thread, several CTAs per
+//     SM): latency is hidden by thread-level parallelism;
 //   * the tensor-product contractions are done by LINE tasks: a thread owns one xi/eta/zeta line of one element,
 //     reads its Nq values from shared memory, applies the full Nq x Nq matrix with D as constant-bank operands
 //     (no D registers) and writes the Nq results back (in place for the divergence);
 //   * face work is a list of 6*Nq^2 FACE tasks per element spread evenly over the CTA's threads; a face whose
 //     neighbour element lives in the same CTA reads the neighbour's state and contravariant flux straight from
 //     shared memory (no global loads, no second EOS / flux evaluation); only CTA-external faces go to L2.
-// Arithmetic, formulas and summation order of the per-node operations are those of cm_dg_kernels.cuh.
+// Parity-tested on all five configs; not tuned (profiles/r1a_v2.md is its only capture).  P:L<n> = paper line.
 #pragma once
 #include "cm_dg_internal.h"
 #include "cm_dg_physics.cuh"
