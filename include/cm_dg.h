@@ -64,6 +64,20 @@ typedef struct {
   double shf_bottom;        /* W m^-2 prescribed upward energy flux through the z-low wall, 0 = none */
 } cm_dg_params;
 
+/* Optional scheduling knobs (HOST, copied by cm_dg_setup_tuned).  They never change what is computed (the parity tests
+ * run every setting against the oracle), only how the work is laid out on the GPU.  All-zero = the defaults, except
+ * ahead_t / ahead_g whose default is -1. */
+typedef struct {
+  int32_t order_lex;     /* 1: lexicographic element order instead of the tiled one (lex_of_elem becomes the identity)   */
+  int32_t max_chunk;     /* tiled order: longest x-chunk L (L divides Ex), 0 = 32                                       */
+  int32_t max_patch;     /* tiled order: tallest y-patch PY (PY divides Ey), 0 = 16                                     */
+  int32_t force_general; /* 1: use the stored-metric kernels (the path of warped meshes) on a flat mesh too             */
+  int32_t kernel;        /* 0 default | 10 row-sweep kernels (flat) | 7 CTA-per-element kernels (flat) | 2 stored-metric */
+  int32_t ahead_t;       /* kernel 7: L2 prefetch distance of the tendency kernel in elements; -1 one wave, 0 off       */
+  int32_t ahead_g;       /* same for the gradient kernel                                                                */
+  int32_t row_len;       /* kernel 10: elements per row sweep (must divide the x-chunk), 0 = the whole chunk            */
+} cm_dg_tuning;
+
 /* Conservation integrals and step-size ingredients (eq. 57; eq. 61-62). */
 typedef struct {
   double mass;          /* sum M rho,        M = w_i w_j w_k |J|                                           */
@@ -87,6 +101,10 @@ typedef struct {
  * reference state.  `cuda_stream` is a cudaStream_t (NULL = default stream).  On success *out owns all
  * device scratch (geometry, gradient array, LSRK residual, two more state buffers). */
 int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out);
+
+/* Same with explicit scheduling knobs (tuning == NULL: defaults).  CM_DG_EINVAL for an unknown kernel id or a row_len
+ * that does not divide the x-chunk. */
+int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tuning, void* cuda_stream, cm_dg_ctx** out);
 
 /* Layout of state arrays: n_elem, np, field_stride (doubles) and, if non-NULL, lex_of_elem (HOST, n_elem
  * int32 entries).  Any output pointer may be NULL. */

@@ -6,7 +6,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIBPATH = os.environ.get("CM_DG_LIB", os.path.join(_HERE, "libcm_dg.so"))   # CM_DG_LIB: a differently tuned build of the same library
+_LIBPATH = os.path.join(_HERE, "libcm_dg.so")
 
 
 class CmDgError(RuntimeError):
@@ -26,6 +26,11 @@ class _Params(C.Structure):
     ]
 
 
+class _Tuning(C.Structure):
+    _fields_ = [("order_lex", C.c_int32), ("max_chunk", C.c_int32), ("max_patch", C.c_int32), ("force_general", C.c_int32),
+                ("kernel", C.c_int32), ("ahead_t", C.c_int32), ("ahead_g", C.c_int32), ("row_len", C.c_int32)]
+
+
 class _Diag(C.Structure):
     _fields_ = [("mass", C.c_double), ("energy", C.c_double), ("water", C.c_double), ("kinetic", C.c_double),
                 ("max_wavespeed", C.c_double), ("min_node_dx", C.c_double), ("volume", C.c_double),
@@ -37,7 +42,7 @@ class _KStats(C.Structure):
                 ("ms_gradient", C.c_double), ("ms_tendency", C.c_double), ("ms_other", C.c_double)]
 
 
-EXPORTS = ("cm_dg_setup", "cm_dg_layout", "cm_dg_coords", "cm_dg_metrics", "cm_dg_gradient", "cm_dg_rhs",
+EXPORTS = ("cm_dg_setup", "cm_dg_setup_tuned", "cm_dg_layout", "cm_dg_coords", "cm_dg_metrics", "cm_dg_gradient", "cm_dg_rhs",
            "cm_dg_lsrk_step", "cm_dg_diagnostics", "cm_dg_rhs_host", "cm_dg_lsrk_step_host",
            "cm_dg_profile_begin", "cm_dg_profile_end", "cm_dg_destroy", "cm_dg_last_error")
 
@@ -58,6 +63,7 @@ def _load():
     L = C.CDLL(_LIBPATH)
     vp, dbl, i32, i64 = C.c_void_p, C.c_double, C.c_int32, C.c_int64
     L.cm_dg_setup.argtypes = [C.POINTER(_Params), vp, C.POINTER(vp)]
+    L.cm_dg_setup_tuned.argtypes = [C.POINTER(_Params), C.POINTER(_Tuning), vp, C.POINTER(vp)]
     L.cm_dg_layout.argtypes = [vp, C.POINTER(i64), C.POINTER(i32), C.POINTER(i64), vp]
     L.cm_dg_coords.argtypes = [vp, vp]
     L.cm_dg_metrics.argtypes = [vp, vp, vp]
@@ -105,8 +111,9 @@ def _hptr(a):
     return C.c_void_p(a.data_ptr())
 
 
-def cm_dg_setup(cfg, stream=None):
-    """cfg: dict with the fields of cm_dg_params (numpy arrays for the HOST pointers).  Returns the ctx handle."""
+def cm_dg_setup(cfg, stream=None, tuning=None):
+    """cfg: dict with the fields of cm_dg_params (numpy arrays for the HOST pointers); tuning: dict with fields of
+    cm_dg_tuning (cm_dg_setup_tuned) or None (cm_dg_setup).  Returns the ctx handle."""
     L = _load()
     p = _Params()
     p.N = int(cfg["N"])
@@ -138,7 +145,15 @@ def cm_dg_setup(cfg, stream=None):
         p.ref_rho = host("ref_rho"); p.ref_rhoe = host("ref_rhoe"); p.ref_rhoq = host("ref_rhoq")
     ctx = C.c_void_p()
     sp = C.c_void_p(int(stream.cuda_stream)) if stream is not None else C.c_void_p(0)
-    _check(L.cm_dg_setup(C.byref(p), sp, C.byref(ctx)), "cm_dg_setup")
+    if tuning is None:
+        _check(L.cm_dg_setup(C.byref(p), sp, C.byref(ctx)), "cm_dg_setup")
+    else:
+        tn = _Tuning(ahead_t=-1, ahead_g=-1)
+        for k, v in tuning.items():
+            if k not in dict(_Tuning._fields_):
+                raise CmDgError("unknown tuning field %r" % k)
+            setattr(tn, k, int(v))
+        _check(L.cm_dg_setup_tuned(C.byref(p), C.byref(tn), sp, C.byref(ctx)), "cm_dg_setup_tuned")
     return ctx
 
 
@@ -202,11 +217,11 @@ def cm_dg_destroy(ctx):
 class CmDg:
     """Owns one ctx; allocates state arrays with torch on the current CUDA device."""
 
-    def __init__(self, cfg, stream=None):
+    def __init__(self, cfg, stream=None, tuning=None):
         import torch
         self.torch = torch
         self.cfg = cfg
-        self.ctx = cm_dg_setup(cfg, stream)
+        self.ctx = cm_dg_setup(cfg, stream, tuning)
         self.n_elem, self.np, self.stride, self.lex_of_elem = cm_dg_layout(self.ctx)
         self.nvar = int(cfg.get("nvar", 5))
         self.device = torch.device("cuda", torch.cuda.current_device())

@@ -25,6 +25,7 @@ struct CmKP {
   // tiled element order e = ((((ey / gPY) * gNXC + ex / gL) * gEz + ez) * gPY + ey % gPY) * gL + ex % gL
   int gL, gPY, gNXC, gNYP, gEz;   // x-chunk length (divides Ex), y-patch height (divides Ey), Ex / gL, Ey / gPY, Ez
   int gbc[3];            // per direction: 1 = walls, 0 = periodic
+  int gS;                // row-sweep kernels: elements per row (divides gL)
   int ahead;             // flat: L2 prefetch distance in elements of the launch order (0 = off)
   float ginvL, ginvNXC;  // 1 / gL, 1 / gNXC (exact small-integer division in cm7_position)
   long long stride;      // field stride in doubles

@@ -554,7 +554,9 @@ __device__ __forceinline__ void cm7_grad_line(const CmKP& p, const double* __res
 }
 
 // RAW: false packed SGS fluxes (hot path) | true the 15 raw gradients (cm_dg_gradient)
-template <int Nq, bool MOIST, bool RAW>
+// GEM: the packed SGS fluxes are stored element-major, G[e][NG][SLOT] (one bulk copy per element for the row-sweep
+// tendency kernel), instead of field-major G[k][stride]
+template <int Nq, bool MOIST, bool RAW, bool GEM = false>
 __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>::MINB_G) cm7_gradient_kernel(const __grid_constant__ CmKP p) {
   using C = CmCfg7<Nq, MOIST>;
   constexpr int NF = C::NF, NP = C::NP, N = Nq - 1, NV = C::NV, NS = C::NS, SLOT = C::SLOT, NFP = C::NFP, THREADS = C::THREADS;
@@ -636,8 +638,8 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
       for (int v = 0; v < NS; ++v) Gr[v][c] *= (p.cA[c] * p.invJ);
     }
     if (!MOIST) { Gr[4][0] = Gr[4][1] = Gr[4][2] = 0.0; }
-    double* o = p.Gout + idx;
-    const long long st = p.stride;
+    double* o = (GEM && !RAW) ? p.Gout + (size_t)e * (C::NG * SLOT) + n : p.Gout + idx;
+    const long long st = (GEM && !RAW) ? (long long)SLOT : p.stride;
     if (RAW) {
 #pragma unroll
       for (int v = 0; v < 5; ++v)
@@ -735,7 +737,7 @@ __device__ __forceinline__ void cm9_grad_line(const CmKP& p, const double* __res
   }
 }
 
-template <int Nq, bool MOIST, bool RAW>
+template <int Nq, bool MOIST, bool RAW, bool GEM = false>
 __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg9<Nq, MOIST>::MINB_G) cm9_gradient_kernel(const __grid_constant__ CmKP p) {
   using C = CmCfg7<Nq, MOIST>;
   constexpr int NF = C::NF, NP = C::NP, N = Nq - 1, NV = C::NV, NS = C::NS, SLOT = C::SLOT, NFP = C::NFP, THREADS = C::THREADS;
@@ -825,8 +827,8 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg9<Nq, MOIST>:
 #pragma unroll
       for (int c = 0; c < 3; ++c) Gr[v][c] = (p.cA[c] * p.invJ) * dd[(c * NS + v) * SLOT + n];
     if (!MOIST) { Gr[4][0] = Gr[4][1] = Gr[4][2] = 0.0; }
-    double* o = p.Gout + idx;
-    const long long st = p.stride;
+    double* o = (GEM && !RAW) ? p.Gout + (size_t)e * (C::NG * SLOT) + n : p.Gout + idx;
+    const long long st = (GEM && !RAW) ? (long long)SLOT : p.stride;
     if (RAW) {
 #pragma unroll
       for (int v = 0; v < 5; ++v)

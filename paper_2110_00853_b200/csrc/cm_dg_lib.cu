@@ -248,13 +248,14 @@ __global__ void diag_kernel(const __grid_constant__ DiagArgs a, double* __restri
 struct cm_dg_ctx {
   cm_dg_params prm;
   int N, Nq, Np, nvar, ngrad, general, moist;
-  int variant = 7;   // 7: CTA-per-element kernels, all inputs staged asynchronously (cm_dg_kernels7.cuh; flat bricks);
-                     // 2: thread-per-node kernels (cm_dg_kernels2.cuh; any geometry); env CM_DG_KERNEL=2 forces the latter
+  int variant = 10;  // 10: row-sweep kernels (cm_dg_kernels10.cuh; flat bricks); 7: CTA-per-element kernels (cm_dg_kernels7.cuh; flat bricks);
+                     // 2: thread-per-node kernels (cm_dg_kernels2.cuh; any geometry); cm_dg_tuning::kernel selects
   int64_t Ne, stride;
   cudaStream_t st;
   std::vector<int32_t> lex_of_elem;
   double xi[CM_MAXNQ], w[CM_MAXNQ], D[CM_MAXNQ][CM_MAXNQ];
   double h[3], min_node_dx;
+  size_t em_bytes_per_field = 0;   // bytes per field of G and of the residual (field-major or element-major layout)
   // device
   int *d_nbr = nullptr, *d_erow = nullptr, *d_lex = nullptr;
   double *d_ztab = nullptr, *d_geo = nullptr, *d_ref = nullptr, *d_G = nullptr, *d_res = nullptr, *d_Q2 = nullptr, *d_Q3 = nullptr;
@@ -341,7 +342,17 @@ const char* cm_dg_last_error(void) { return g_err.c_str(); }
 void cm_dg_destroy(cm_dg_ctx* ctx) { free_ctx(ctx); }
 
 int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
+  return cm_dg_setup_tuned(p, nullptr, cuda_stream, out);
+}
+
+int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cuda_stream, cm_dg_ctx** out) {
   if (!p || !out) return fail(CM_DG_EINVAL, "cm_dg_setup: NULL argument");
+  cm_dg_tuning tn;
+  std::memset(&tn, 0, sizeof(tn));
+  tn.ahead_t = tn.ahead_g = -1;
+  if (tune) tn = *tune;
+  if (tn.kernel != 0 && tn.kernel != 2 && tn.kernel != 7 && tn.kernel != 10) return fail(CM_DG_EINVAL, "cm_dg_setup_tuned: kernel must be 0, 2, 7 or 10");
+  if (tn.max_chunk < 0 || tn.max_patch < 0 || tn.row_len < 0) return fail(CM_DG_EINVAL, "cm_dg_setup_tuned: negative tile size");
   *out = nullptr;
   if (p->N < 2 || p->N > 7) return fail(CM_DG_EINVAL, "cm_dg_setup: polynomial order N must be in 2..7");
   if (p->nvar != 5 && p->nvar != 6) return fail(CM_DG_EINVAL, "cm_dg_setup: nvar must be 5 or 6");
@@ -384,11 +395,8 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   // neighbour at most Ez*PY*L).  The flat kernels recompute this map from blockIdx (cm6_position).
   int L = 1, PY = 1;
   {
-    const char* ord = std::getenv("CM_DG_ORDER");
-    const bool lex_order = ord && std::strcmp(ord, "lex") == 0;
-    int maxL = 32, maxPY = 16;
-    if (const char* sl = std::getenv("CM_DG_SEGLEN")) { const int v = std::atoi(sl); if (v >= 1) maxL = v; }
-    if (const char* py = std::getenv("CM_DG_PATCH")) { const int v = std::atoi(py); if (v >= 1) maxPY = v; }
+    const bool lex_order = tn.order_lex != 0;
+    const int maxL = tn.max_chunk > 0 ? tn.max_chunk : 32, maxPY = tn.max_patch > 0 ? tn.max_patch : 16;
     for (int d = 1; d <= p->ne[0] && d <= maxL; ++d) if (p->ne[0] % d == 0) L = d;
     for (int d = 1; d <= p->ne[1] && d <= maxPY; ++d) if (p->ne[1] % d == 0) PY = d;
     if (lex_order) { L = p->ne[0]; PY = p->ne[1]; }
@@ -438,8 +446,8 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
       }
   }
   c->general = (p->geom != 0 || (p->use_ref && !ref_z_only)) ? 1 : 0;
-  if (const char* fg = std::getenv("CM_DG_FORCE_GENERAL")) if (fg[0] == '1') c->general = 1;
-  if (const char* kv = std::getenv("CM_DG_KERNEL")) if (kv[0] == '2' || kv[0] == '7') c->variant = kv[0] - '0';
+  if (tn.force_general) c->general = 1;
+  if (tn.kernel) c->variant = tn.kernel;
   if (c->general) c->variant = 2;
 
   auto bail = [&](int code) { free_ctx(c); return code; };
@@ -479,9 +487,13 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   kp.ginvL = 1.0f / (float)L; kp.ginvNXC = 1.0f / (float)(p->ne[0] / L);
   kp.gL = L; kp.gPY = PY; kp.gNXC = p->ne[0] / L; kp.gNYP = p->ne[1] / PY; kp.gEz = p->ne[2];
   for (int d = 0; d < 3; ++d) kp.gbc[d] = p->bc[d];
-  kp.ahead = -1;   // L2 prefetch distance: -1 = one wave of resident CTAs (set by the launcher); CM_DG_AHEAD_T / _G override
-  if (const char* ah = std::getenv("CM_DG_AHEAD_T")) c->ahead_t = std::atoi(ah);
-  if (const char* ah = std::getenv("CM_DG_AHEAD_G")) c->ahead_g = std::atoi(ah);
+  kp.ahead = -1;   // L2 prefetch distance of the cm7 kernels: -1 = one wave of resident CTAs (set by the launcher)
+  c->ahead_t = tn.ahead_t; c->ahead_g = tn.ahead_g;
+  kp.gS = L;       // row-sweep kernels: a row is a whole x-chunk unless the tuning asks for shorter rows
+  if (tn.row_len > 0) {
+    if (L % tn.row_len != 0) { fail(CM_DG_EINVAL, "cm_dg_setup_tuned: row_len must divide the x-chunk length"); return bail(CM_DG_EINVAL); }
+    kp.gS = tn.row_len;
+  }
   if ((int64_t)PY * L > 2147483647LL || p->ne[2] > 65535 || (int64_t)kp.gNXC * kp.gNYP > 65535) {
     fail(CM_DG_EINVAL, "cm_dg_setup: mesh exceeds the launch-grid limits (Ez and (Ex/L)*(Ey/PY) must be <= 65535)");
     return bail(CM_DG_EINVAL);
@@ -565,7 +577,10 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
   (void)nn;
 
   // ---- scratch owned by the ctx
-  if (p->sgs) CM_CUDA_B(cudaMalloc(&c->d_G, (size_t)c->ngrad * fbytes));
+  // element-major internal arrays of the row-sweep kernels: [e][field][SLOT], SLOT = Np rounded up to even
+  const size_t slot = (size_t)Np + (Np & 1);
+  c->em_bytes_per_field = std::max(fbytes, (size_t)Ne * slot * sizeof(double));
+  if (p->sgs) CM_CUDA_B(cudaMalloc(&c->d_G, (size_t)c->ngrad * c->em_bytes_per_field));
   CM_CUDA_B(cudaMalloc(&c->d_part, (size_t)Ne * 7 * sizeof(double)));
   // residual and ping-pong state are allocated on first use by cm_dg_lsrk_step
 
@@ -629,7 +644,7 @@ int cm_dg_lsrk_step(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t 
   if (!ctx || !Q_dev) return fail(CM_DG_EINVAL, "cm_dg_lsrk_step: NULL argument");
   if (nsteps < 0) return fail(CM_DG_EINVAL, "cm_dg_lsrk_step: nsteps must be >= 0");
   const size_t bytes = (size_t)ctx->nvar * ctx->stride * sizeof(double);
-  if (!ctx->d_res) CM_CUDA(cudaMalloc(&ctx->d_res, bytes));
+  if (!ctx->d_res) CM_CUDA(cudaMalloc(&ctx->d_res, (size_t)ctx->nvar * ctx->em_bytes_per_field));
   if (!ctx->d_Q2) { CM_CUDA(cudaMalloc(&ctx->d_Q2, bytes)); CM_CUDA(cudaMemsetAsync(ctx->d_Q2, 0, bytes, ctx->st)); }
   if (!ctx->d_Q3) { CM_CUDA(cudaMalloc(&ctx->d_Q3, bytes)); CM_CUDA(cudaMemsetAsync(ctx->d_Q3, 0, bytes, ctx->st)); }
   // A stage never updates in place (neighbours still read the old state).  Three buffers in the cycle

@@ -18,8 +18,8 @@ def P():
     return pkg
 
 
-def _pair(P, oracle_mod, cfg):
-    return oracle_mod.Oracle(cfg), P.CmDg(cfg)
+def _pair(P, oracle_mod, cfg, tuning=None):
+    return oracle_mod.Oracle(cfg), P.CmDg(cfg, tuning=tuning)
 
 
 @pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
@@ -68,28 +68,30 @@ def test_rhs_parity(P, oracle_mod, k, N):
         assert np.all(err <= RHS_TOL), (label, err)
 
 
-def test_rhs_parity_general_path_on_flat_mesh(P, oracle_mod, monkeypatch):
+def test_rhs_parity_general_path_on_flat_mesh(P, oracle_mod):
     """The stored-metric kernels must agree with the oracle on a flat mesh too (moist + SGS + walls)."""
-    monkeypatch.setenv("CM_DG_FORCE_GENERAL", "1")
     cfg, Q, dt = small_config(5)
-    o, g = _pair(P, oracle_mod, cfg)
+    o, g = _pair(P, oracle_mod, cfg, tuning={"force_general": 1})
     Q = o.lsrk54(Q, dt, 2)
     err = rhs_errors(g.to_host(g.rhs(g.to_device(Q))), o.rhs(Q), cfg, Q, o.diagnostics(Q)["min_node_dx"])
     assert np.all(err <= RHS_TOL), err
 
 
-@pytest.mark.parametrize("env", [{"CM_DG_SEGLEN": "1"}, {"CM_DG_SEGLEN": "2", "CM_DG_PATCH": "2"}, {"CM_DG_SEGLEN": "3", "CM_DG_PATCH": "3"},
-                                 {"CM_DG_KERNEL": "2"}, {"CM_DG_AHEAD_T": "1", "CM_DG_AHEAD_G": "2"},
-                                 {"CM_DG_AHEAD_T": "0", "CM_DG_AHEAD_G": "0"}])
+@pytest.mark.parametrize("tuning", [{"max_chunk": 1}, {"max_chunk": 2, "max_patch": 2}, {"max_chunk": 3, "max_patch": 3},
+                                    {"row_len": 1}, {"row_len": 2, "max_chunk": 4}, {"kernel": 2},
+                                    {"kernel": 7}, {"kernel": 7, "max_chunk": 2, "max_patch": 2},
+                                    {"kernel": 7, "ahead_t": 1, "ahead_g": 2}, {"kernel": 7, "ahead_t": 0, "ahead_g": 0}],
+                         ids=lambda d: ",".join("%s=%s" % kv for kv in d.items()))
 @pytest.mark.parametrize("k", [1, 3, 5])
-def test_parity_schedule_variants(P, oracle_mod, monkeypatch, env, k):
-    """Tile shape of the element order (x-chunk length / y-patch height, i.e. the launch grid of the flat kernels), the
-    thread-per-node kernels on flat meshes, and the L2 prefetch distance (small meshes are shorter than one wave, so the
-    default distance never prefetches there): RHS and 7 fused steps against the oracle."""
-    for key, val in env.items():
-        monkeypatch.setenv(key, val)
+def test_parity_schedule_variants(P, oracle_mod, tuning, k):
+    """cm_dg_tuning: tile shape of the element order (x-chunk length / y-patch height, i.e. the launch grid of the flat
+    kernels), row length of the row-sweep kernels, the CTA-per-element and the thread-per-node kernels on flat meshes,
+    and the L2 prefetch distance (small meshes are shorter than one wave, so the default distance never prefetches
+    there): RHS and 7 fused steps against the oracle."""
     cfg, Q, dt = small_config(k)
-    o, g = _pair(P, oracle_mod, cfg)
+    if "row_len" in tuning and cfg["ne"][0] % max(tuning["row_len"], tuning.get("max_chunk", 1)) != 0:
+        pytest.skip("row length does not divide this mesh")
+    o, g = _pair(P, oracle_mod, cfg, tuning=tuning)
     Q1 = o.lsrk54(Q, dt, 2)
     err = rhs_errors(g.to_host(g.rhs(g.to_device(Q1))), o.rhs(Q1), cfg, Q1, o.diagnostics(Q1)["min_node_dx"])
     assert np.all(err <= RHS_TOL), err
@@ -99,10 +101,9 @@ def test_parity_schedule_variants(P, oracle_mod, monkeypatch, env, k):
     assert np.all(err <= STEP_TOL), err
 
 
-def test_rhs_parity_lexicographic_order(P, oracle_mod, monkeypatch):
-    monkeypatch.setenv("CM_DG_ORDER", "lex")
+def test_rhs_parity_lexicographic_order(P, oracle_mod):
     cfg, Q, dt = small_config(3)
-    o, g = _pair(P, oracle_mod, cfg)
+    o, g = _pair(P, oracle_mod, cfg, tuning={"order_lex": 1})
     assert np.all(g.lex_of_elem == np.arange(o.Ne))
     err = rhs_errors(g.to_host(g.rhs(g.to_device(Q))), o.rhs(Q), cfg, Q, o.diagnostics(Q)["min_node_dx"])
     assert np.all(err <= RHS_TOL), err
