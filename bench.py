@@ -189,7 +189,7 @@ def run_ours(args):
     cfg, Q, dt = cut_of_config5(args.ne, args.order)
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
-        g = P.CmDg(cfg, stream=stream)
+        g = P.CmDg(cfg, stream=stream, tuning=args.tuning)
         Qh = torch.from_numpy(g.pack(Q)).pin_memory()
         del Q
         Qd = Qh.to(g.device, non_blocking=True)
@@ -296,7 +296,11 @@ def main():
     ap.add_argument("--ne", type=int, nargs=3, default=None, help="element counts (default: the full config-5 mesh)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tuning", nargs="*", default=None, metavar="KEY=VAL",
+                    help="cm_dg_tuning fields for kernel experiments (e.g. kernel=7 row_len=16); default: the library's defaults")
     args = ap.parse_args()
+    if args.tuning is not None:
+        args.tuning = {kv.split("=")[0]: int(kv.split("=")[1]) for kv in args.tuning} or None
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     import workloads as W

@@ -432,3 +432,4 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS + 32, CmCfg10<Nq, M
     }
   }
 }
+

@@ -76,6 +76,9 @@ __device__ __forceinline__ void cm7_cp_commit() { asm volatile("cp.async.commit_
 __device__ __forceinline__ void cm7_cp_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void cm7_cp_wait_but_one() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 
+#ifndef CM_LINE_UNROLL
+#define CM_LINE_UNROLL 3   // variables per unrolled body of the tendency line task (code size vs ILP: profiles/r2_rowsweep.md)
+#endif
 #define CM_ZSM_W 10   // doubles per z-table row in shared memory (CmCfg7::ZW)
 
 template <int Nq, bool MOIST> struct CmCfg7 {
@@ -332,7 +335,8 @@ __device__ __forceinline__ void cm7_tend_line(const CmKP& p, double* __restrict_
   constexpr int N = Nq - 1;
   const double c0 = p.inv_w0 * (((wallmask >> (2 * D)) & 1) ? 1.0 : 0.5);      // -sgn = +1 at the low end
   const double cN = -p.inv_w0 * (((wallmask >> (2 * D + 1)) & 1) ? 1.0 : 0.5);
-#pragma unroll
+  constexpr int LU = CM_LINE_UNROLL;
+#pragma unroll LU
   for (int v = 0; v < NV; ++v) {
     double* q = q0 + v * TSL;
     double x[Nq], y[Nq];
