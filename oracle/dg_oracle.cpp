@@ -159,11 +159,14 @@ void elem_geo_compute(const Ctx& c, int64_t e, double* x, double* Ja, double* J)
       for (int i = 0; i < Nq; ++i) {
         int n = i + Nq * (j + Nq * k);
         double xr[3] = {0, 0, 0}, xs[3] = {0, 0, 0}, xt[3] = {0, 0, 0};  // d(x,y,z)/dxi, /deta, /dzeta
+        // The coordinates are differentiated relative to the element's first node: D annihilates constants, so this is
+        // eq. (24) unchanged, but the products D_im * x_m no longer carry the element's offset from the origin (up to
+        // 3e5 m), whose rounding left spurious off-diagonal metric terms of relative size 8 eps |x| / h ~ 1e-13.
         for (int m = 0; m < Nq; ++m)
           for (int d = 0; d < 3; ++d) {
-            xr[d] += c.D[i][m] * x[3 * (m + Nq * (j + Nq * k)) + d];
-            xs[d] += c.D[j][m] * x[3 * (i + Nq * (m + Nq * k)) + d];
-            xt[d] += c.D[k][m] * x[3 * (i + Nq * (j + Nq * m)) + d];
+            xr[d] += c.D[i][m] * (x[3 * (m + Nq * (j + Nq * k)) + d] - x[d]);
+            xs[d] += c.D[j][m] * (x[3 * (i + Nq * (m + Nq * k)) + d] - x[d]);
+            xt[d] += c.D[k][m] * (x[3 * (i + Nq * (j + Nq * m)) + d] - x[d]);
           }
         double* a = Ja + 9 * n;
         // Ja^1 = x_eta x x_zeta ; Ja^2 = x_zeta x x_xi ; Ja^3 = x_xi x x_eta

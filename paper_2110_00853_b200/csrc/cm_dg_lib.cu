@@ -135,11 +135,12 @@ __global__ void metrics_kernel(const __grid_constant__ GeoArgs a, double* __rest
   for (int n = threadIdx.x; n < Np; n += blockDim.x) {
     const int i = n % Nq, j = (n / Nq) % Nq, k = n / (Nq * Nq);
     double xr[3] = {0, 0, 0}, xs[3] = {0, 0, 0}, xt[3] = {0, 0, 0};
+    // coordinates relative to the element's first node: same derivative, no rounding of the offset from the origin
     for (int m = 0; m < Nq; ++m)
       for (int d = 0; d < 3; ++d) {
-        xr[d] += a.D[i][m] * X[d * Np + m + Nq * (j + Nq * k)];
-        xs[d] += a.D[j][m] * X[d * Np + i + Nq * (m + Nq * k)];
-        xt[d] += a.D[k][m] * X[d * Np + i + Nq * (j + Nq * m)];
+        xr[d] += a.D[i][m] * (X[d * Np + m + Nq * (j + Nq * k)] - X[d * Np]);
+        xs[d] += a.D[j][m] * (X[d * Np + i + Nq * (m + Nq * k)] - X[d * Np]);
+        xt[d] += a.D[k][m] * (X[d * Np + i + Nq * (j + Nq * m)] - X[d * Np]);
       }
     double A[9];
     A[0] = xs[1] * xt[2] - xs[2] * xt[1]; A[1] = xs[2] * xt[0] - xs[0] * xt[2]; A[2] = xs[0] * xt[1] - xs[1] * xt[0];

@@ -10,6 +10,9 @@ template <int Nq> struct CmNodes {
 
 // 1/a and sqrt(a) to ~1 ulp from the MUFU seed plus two Newton steps: no slow-path branches (a > 0 here).
 __device__ __forceinline__ double cm_rcp(double a) {
+#ifdef CM_EXACT_MATH
+  return 1.0 / a;
+#endif
   double x;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(a));
   double e = fma(-a, x, 1.0); x = fma(x, e, x);
@@ -17,6 +20,13 @@ __device__ __forceinline__ double cm_rcp(double a) {
   return x;
 }
 __device__ __forceinline__ double cm_sqrt(double a) {
+  // the MUFU seed flushes subnormal inputs to zero (-> inf -> NaN after the Newton steps): squared strain rates of a
+  // flow that has barely started (edge of the thermal bubble after one stage) do underflow that far, so arguments below
+  // the fast path's safe range take the IEEE routine.  Rare, warp-uniform in practice.
+  if (a < 1e-280) return (a > 0.0) ? sqrt(a) : 0.0;
+#ifdef CM_EXACT_MATH
+  return sqrt(a);
+#endif
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
   double r = a * y, h = 0.5 * y;
