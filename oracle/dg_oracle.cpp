@@ -15,7 +15,11 @@
 //   O8  Rusanov flux (eq. 27), central flux for F2, walls (App. A)
 //   O9  LSRK54 (Carpenter & Kennedy 1994, cited P:L286) and forward Euler
 //   O10 diagnostics: eq. (57), (61)-(62) P:L587-591
-// Readings of the paper where it is silent or garbled are R1..R23 of DESIGN.md.
+//   O11 Vreman eddy viscosity (eq. 39a-d) and the Richardson stability factor (eq. 40)
+//   O12 Rayleigh sponge (eq. A4-A5) and the exponential element filter (eq. 52)
+//   O13 any 2N-storage LSRK coefficient table, HLLC flux (named P:L256; Toro et al. 1994, textbook form),
+//       curl-invariant metric terms (Kopriva 2006) for fully 3-D warps
+// Readings of the paper where it is silent or garbled are R1..R29 of DESIGN.md.
 //
 // Data layout of the oracle (deliberately NOT the GPU layout): array-of-structures,
 //   Q[e][n][v], e = ex + Ex*(ey + Ey*ez) lexicographic, n = i + Nq*(j + Nq*k), v = rho,rhou,rhov,rhow,rhoe,[rhoq].
@@ -54,11 +58,21 @@ struct Ctx {
   int use_ref;
   std::vector<double> ref_rho, ref_rhoe, ref_rhoq;  // [Ne][Np]
   double shf_bottom;
+  int richardson = 0;              // eq. (40) on / off
+  double p_0 = 1.0e5;              // reference pressure of theta_v (R25)
+  double sponge_alpha = 0.0, sponge_zs = 0.0; int sponge_gamma = 2; double u_relax[3] = {0, 0, 0};   // eq. (A4)-(A5)
+  int filter_order = 0; double filter_alpha = 36.0436533891172;   // eq. (52); alpha = -log(2^-52)
+  int riemann = 0;                 // 0 Rusanov (eq. 27) | 1 HLLC
+  int metric_form = 0;             // 0 cross-product (R4) | 1 curl-invariant
   double xi[MAXNQ], w[MAXNQ], D[MAXNQ][MAXNQ];
+  double Filt[MAXNQ][MAXNQ];       // 1-D nodal filter matrix V diag(sigma) V^-1
   // optional cache of per-element geometry (same function fills it; see elem_geo)
   bool cached = false;
-  std::vector<double> cx, cJa, cJ;
+  std::vector<double> cx, cJa, cJ, cDx;
 };
+
+constexpr int NGV = 6;             // gradient variables u, v, w, h_tot, q_t, theta_v
+constexpr int NG3 = 3 * NGV;
 
 // ---------------------------------------------------------------- O1: 1-D operators
 void legendre(int N, double x, double& P, double& dP) {
@@ -151,9 +165,10 @@ void elem_nodes(const Ctx& c, int64_t e, double* x) {
 }
 
 // Geometry of one element: x[n][3]; Ja[n][d][cc] = J * d(xi_d)/d(x_cc) (cross-product form); J[n] = det(dx/dxi).
-void elem_geo_compute(const Ctx& c, int64_t e, double* x, double* Ja, double* J) {
+void elem_geo_compute(const Ctx& c, int64_t e, double* x, double* Ja, double* J, double* dxd) {
   const int Nq = c.Nq, Np = c.Np;
   elem_nodes(c, e, x);
+  std::vector<double> dX(9 * (size_t)Np);   // dX[n][d][cc] = d x_cc / d xi_d
   for (int k = 0; k < Nq; ++k)
     for (int j = 0; j < Nq; ++j)
       for (int i = 0; i < Nq; ++i) {
@@ -168,28 +183,58 @@ void elem_geo_compute(const Ctx& c, int64_t e, double* x, double* Ja, double* J)
             xs[d] += c.D[j][m] * (x[3 * (i + Nq * (m + Nq * k)) + d] - x[d]);
             xt[d] += c.D[k][m] * (x[3 * (i + Nq * (j + Nq * m)) + d] - x[d]);
           }
+        for (int d = 0; d < 3; ++d) { dX[9 * n + d] = xr[d]; dX[9 * n + 3 + d] = xs[d]; dX[9 * n + 6 + d] = xt[d]; }
         double* a = Ja + 9 * n;
         // Ja^1 = x_eta x x_zeta ; Ja^2 = x_zeta x x_xi ; Ja^3 = x_xi x x_eta
         a[0] = xs[1] * xt[2] - xs[2] * xt[1]; a[1] = xs[2] * xt[0] - xs[0] * xt[2]; a[2] = xs[0] * xt[1] - xs[1] * xt[0];
         a[3] = xt[1] * xr[2] - xt[2] * xr[1]; a[4] = xt[2] * xr[0] - xt[0] * xr[2]; a[5] = xt[0] * xr[1] - xt[1] * xr[0];
         a[6] = xr[1] * xs[2] - xr[2] * xs[1]; a[7] = xr[2] * xs[0] - xr[0] * xs[2]; a[8] = xr[0] * xs[1] - xr[1] * xs[0];
         J[n] = xr[0] * a[0] + xr[1] * a[1] + xr[2] * a[2];
+        dxd[3 * n + 0] = xr[0]; dxd[3 * n + 1] = xs[1]; dxd[3 * n + 2] = xt[2];   // diagonal of dx/dxi: mixing lengths (eq. 39)
       }
+  if (c.metric_form == 1) {
+    // Curl-invariant form (Kopriva 2006): Ja^i_n = -xhat_i . curl_xi( I_N( X_l grad_xi X_m ) ), (n, m, l) cyclic.  The
+    // products are interpolated (taken at the nodes) BEFORE the outer derivative, so sum_i d(Ja^i_n)/d xi_i = 0 holds
+    // discretely on any mesh (D_eta D_zeta commute), which the cross-product form only does on extruded meshes (R4).
+    std::vector<double> V(3 * (size_t)Np);   // V[n][d] = X_l * d X_m / d xi_d
+    for (int nn = 0; nn < 3; ++nn) {
+      const int mm = (nn + 1) % 3, ll = (nn + 2) % 3;
+      for (int n = 0; n < Np; ++n)
+        for (int d = 0; d < 3; ++d) V[3 * n + d] = (x[3 * n + ll] - x[ll]) * dX[9 * n + 3 * d + mm];
+      for (int k = 0; k < Nq; ++k)
+        for (int j = 0; j < Nq; ++j)
+          for (int i = 0; i < Nq; ++i) {
+            int n = i + Nq * (j + Nq * k);
+            double dV[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};   // dV[a][d] = d V_d / d xi_a
+            for (int m = 0; m < Nq; ++m)
+              for (int d = 0; d < 3; ++d) {
+                dV[0][d] += c.D[i][m] * V[3 * (m + Nq * (j + Nq * k)) + d];
+                dV[1][d] += c.D[j][m] * V[3 * (i + Nq * (m + Nq * k)) + d];
+                dV[2][d] += c.D[k][m] * V[3 * (i + Nq * (j + Nq * m)) + d];
+              }
+            // curl components: (d_eta V_3 - d_zeta V_2, d_zeta V_1 - d_xi V_3, d_xi V_2 - d_eta V_1)
+            Ja[9 * n + 0 + nn] = -(dV[1][2] - dV[2][1]);
+            Ja[9 * n + 3 + nn] = -(dV[2][0] - dV[0][2]);
+            Ja[9 * n + 6 + nn] = -(dV[0][1] - dV[1][0]);
+          }
+    }
+  }
 }
 
 struct Geo {  // views for one element
-  const double *x, *Ja, *J;
-  std::vector<double> sx, sJa, sJ;
+  const double *x, *Ja, *J, *dxd;
+  std::vector<double> sx, sJa, sJ, sDx;
 };
 void elem_geo(const Ctx& c, int64_t e, Geo& g) {
   const int Np = c.Np;
   if (c.cached) {
     g.x = &c.cx[(size_t)e * Np * 3]; g.Ja = &c.cJa[(size_t)e * Np * 9]; g.J = &c.cJ[(size_t)e * Np];
+    g.dxd = &c.cDx[(size_t)e * Np * 3];
     return;
   }
-  g.sx.resize(3 * Np); g.sJa.resize(9 * Np); g.sJ.resize(Np);
-  elem_geo_compute(c, e, g.sx.data(), g.sJa.data(), g.sJ.data());
-  g.x = g.sx.data(); g.Ja = g.sJa.data(); g.J = g.sJ.data();
+  g.sx.resize(3 * Np); g.sJa.resize(9 * Np); g.sJ.resize(Np); g.sDx.resize(3 * Np);
+  elem_geo_compute(c, e, g.sx.data(), g.sJa.data(), g.sJ.data(), g.sDx.data());
+  g.x = g.sx.data(); g.Ja = g.sJa.data(); g.J = g.sJ.data(); g.dxd = g.sDx.data();
 }
 
 // neighbour across face f (0..5 = -xi,+xi,-eta,+eta,-zeta,+zeta); -1 if the face is a wall.
@@ -219,7 +264,7 @@ inline int face_node(int Nq, int f, int a, int b, bool other_side) {
 
 // ---------------------------------------------------------------- O3: thermodynamics at a node
 struct Prim {
-  double rho, u[3], q, K, Phi, T, p, pp /* p - p_r */, htot, c, rho_r;
+  double rho, u[3], q, K, Phi, T, p, pp /* p - p_r */, htot, c, rho_r, theta_v;
 };
 
 Prim primitives(const Ctx& c, const double* Y, double z, bool has_ref, double rr, double rer, double rqr) {
@@ -236,6 +281,8 @@ Prim primitives(const Ctx& c, const double* Y, double z, bool has_ref, double rr
   P.p = P.rho * Rm * P.T;                                               // eq. (13)
   P.htot = Y[4] / Y[0] + Rm * P.T;                                      // (rho e + p)/rho
   P.c = std::sqrt((1.0 + Rm / cvm) * Rm * P.T);
+  // virtual potential temperature without condensate (R25): theta_v = T (R_m / R_d) (p_0 / p)^(R_d / c_pd)
+  P.theta_v = P.T * (Rm / c.R_d) * std::pow(c.p_0 / P.p, c.R_d / (c.c_vd + c.R_d));
   P.rho_r = 0.0;
   if (has_ref) {
     // R12: p - p_r evaluated from state differences (exact identity for the EOS above, with
@@ -265,9 +312,9 @@ inline Prim prim_at(const Ctx& c, const double* Q, int64_t e, int n, double z) {
   return primitives(c, Y, z, false, 0, 0, 0);
 }
 
-// gradient variables s = (u, v, w, h_tot, q_t)   (eq. 33, 35, 37)
+// gradient variables s = (u, v, w, h_tot, q_t, theta_v)   (eq. 33, 35, 37, 40)
 inline void grad_vars(const Prim& P, double* s) {
-  s[0] = P.u[0]; s[1] = P.u[1]; s[2] = P.u[2]; s[3] = P.htot; s[4] = P.q;
+  s[0] = P.u[0]; s[1] = P.u[1]; s[2] = P.u[2]; s[3] = P.htot; s[4] = P.q; s[5] = P.theta_v;
 }
 
 // ---------------------------------------------------------------- O4: BR1 gradient of one element
@@ -275,26 +322,26 @@ inline void grad_vars(const Prim& P, double* s) {
 void gradient_element(const Ctx& c, const double* Q, int64_t e, double* G) {
   const int Nq = c.Nq, Np = c.Np;
   Geo g; elem_geo(c, e, g);
-  std::vector<double> s(5 * Np);
+  std::vector<double> s(NGV * Np);
   for (int n = 0; n < Np; ++n) {
     Prim P = prim_at(c, Q, e, n, g.x[3 * n + 2]);
-    grad_vars(P, &s[5 * n]);
+    grad_vars(P, &s[NGV * n]);
   }
   // volume part: G_cc = sum_d (Ja^d_cc / J) (D_d s)      (eq. 24, 28)
   for (int k = 0; k < Nq; ++k)
     for (int j = 0; j < Nq; ++j)
       for (int i = 0; i < Nq; ++i) {
         int n = i + Nq * (j + Nq * k);
-        for (int v = 0; v < 5; ++v) {
+        for (int v = 0; v < NGV; ++v) {
           double dr = 0, ds = 0, dt = 0;
           for (int m = 0; m < Nq; ++m) {
-            dr += c.D[i][m] * s[5 * (m + Nq * (j + Nq * k)) + v];
-            ds += c.D[j][m] * s[5 * (i + Nq * (m + Nq * k)) + v];
-            dt += c.D[k][m] * s[5 * (i + Nq * (j + Nq * m)) + v];
+            dr += c.D[i][m] * s[NGV * (m + Nq * (j + Nq * k)) + v];
+            ds += c.D[j][m] * s[NGV * (i + Nq * (m + Nq * k)) + v];
+            dt += c.D[k][m] * s[NGV * (i + Nq * (j + Nq * m)) + v];
           }
           const double* a = g.Ja + 9 * n;
           for (int cc = 0; cc < 3; ++cc)
-            G[(n * 5 + v) * 3 + cc] = (a[0 + cc] * dr + a[3 + cc] * ds + a[6 + cc] * dt) / g.J[n];
+            G[(n * NGV + v) * 3 + cc] = (a[0 + cc] * dr + a[3 + cc] * ds + a[6 + cc] * dt) / g.J[n];
         }
       }
   // surface part: + (sJ/(w_0 J)) n_cc (s* - s^-)            (eq. 30 with central s*)
@@ -309,21 +356,21 @@ void gradient_element(const Ctx& c, const double* Q, int64_t e, double* G) {
         double sJ = std::sqrt(Ja[0] * Ja[0] + Ja[1] * Ja[1] + Ja[2] * Ja[2]);
         double nrm[3] = {sgn * Ja[0] / sJ, sgn * Ja[1] / sJ, sgn * Ja[2] / sJ};
         double lift = sJ / (c.w[0] * g.J[n]);
-        double sm[5], sstar[5];
-        for (int v = 0; v < 5; ++v) sm[v] = s[5 * n + v];
+        double sm[NGV], sstar[NGV];
+        for (int v = 0; v < NGV; ++v) sm[v] = s[NGV * n + v];
         if (en >= 0) {
           int nn = face_node(Nq, f, a_, b, true);
           Prim Pp = prim_at(c, Q, en, nn, gn.x[3 * nn + 2]);
-          double sp[5]; grad_vars(Pp, sp);
-          for (int v = 0; v < 5; ++v) sstar[v] = 0.5 * (sm[v] + sp[v]);
+          double sp[NGV]; grad_vars(Pp, sp);
+          for (int v = 0; v < NGV; ++v) sstar[v] = 0.5 * (sm[v] + sp[v]);
         } else {
           // wall: u_bc = u^- - (n.u^-) n (A6); scalars chi_bc = chi^- (homogeneous Neumann, A8)
           double un = sm[0] * nrm[0] + sm[1] * nrm[1] + sm[2] * nrm[2];
           for (int v = 0; v < 3; ++v) sstar[v] = sm[v] - un * nrm[v];
-          sstar[3] = sm[3]; sstar[4] = sm[4];
+          sstar[3] = sm[3]; sstar[4] = sm[4]; sstar[5] = sm[5];
         }
-        for (int v = 0; v < 5; ++v)
-          for (int cc = 0; cc < 3; ++cc) G[(n * 5 + v) * 3 + cc] += lift * nrm[cc] * (sstar[v] - sm[v]);
+        for (int v = 0; v < NGV; ++v)
+          for (int cc = 0; cc < 3; ++cc) G[(n * NGV + v) * 3 + cc] += lift * nrm[cc] * (sstar[v] - sm[v]);
       }
   }
 }
@@ -339,20 +386,53 @@ void flux_first_order(const Ctx& c, const double* Y, const Prim& P, double (*F)[
   }
 }
 
-// Smagorinsky-Lilly eddy viscosity (eq. 38) with Delta = (8 J)^(1/3) / N (R7).
-double eddy_viscosity(const Ctx& c, const double* G, double J) {
+// Eddy viscosity at a node.  G[s][cc] = d s / d x_cc for s = u, v, w, h_tot, q, theta_v; dxd = diagonal of dx/dxi.
+//   sgs = 1  Smagorinsky-Lilly (eq. 38) with Delta = (8 J)^(1/3) / N (R7)
+//   sgs = 2  Vreman (eq. 39a-d) with the mixing lengths Delta_m = 2 |d x_m / d xi_m| / N (= L_m / N on bricks; R24)
+//   richardson: nu_t is multiplied by f_b of eq. (40), Ri = (g / theta_v) (d theta_v / dz) / |S|^2, |S|^2 = 2 S_ij S_ij
+double eddy_viscosity(const Ctx& c, const double* G, double J, const double* dxd, double theta_v) {
   double S[3][3];
   for (int i = 0; i < 3; ++i)
     for (int j = 0; j < 3; ++j) S[i][j] = 0.5 * (G[i * 3 + j] + G[j * 3 + i]);   // eq. (33); G[s][cc]=d u_s/d x_cc
   double ss = 0;
   for (int i = 0; i < 3; ++i)
     for (int j = 0; j < 3; ++j) ss += S[i][j] * S[i][j];
-  double Delta = std::cbrt(8.0 * J) / c.N;
-  return (c.C_s * Delta) * (c.C_s * Delta) * std::sqrt(2.0 * ss);
+  double nu;
+  if (c.sgs == 2) {
+    double beta[3][3], aa = 0;
+    for (int i = 0; i < 3; ++i)
+      for (int j = 0; j < 3; ++j) {
+        double b = 0;
+        for (int m = 0; m < 3; ++m) {
+          double Dm = 2.0 * std::fabs(dxd[m]) / c.N;
+          b += Dm * Dm * G[i * 3 + m] * G[j * 3 + m];                              // eq. (39c)
+        }
+        beta[i][j] = b;
+        aa += G[i * 3 + j] * G[i * 3 + j];                                         // u_ij u_ij
+      }
+    double B = beta[0][0] * beta[1][1] + beta[0][0] * beta[2][2] + beta[1][1] * beta[2][2] -
+               (beta[0][2] * beta[0][2] + beta[0][1] * beta[0][1] + beta[1][2] * beta[1][2]);   // eq. (39b)
+    nu = (aa > 0.0 && B > 0.0) ? 2.5 * c.C_s * c.C_s * std::sqrt(B / aa) : 0.0;    // eq. (39a); 0/0 := 0 (no flow, no mixing)
+  } else {
+    double Delta = std::cbrt(8.0 * J) / c.N;
+    nu = (c.C_s * Delta) * (c.C_s * Delta) * std::sqrt(2.0 * ss);
+  }
+  if (c.richardson) {
+    double N2 = (c.grav / theta_v) * G[5 * 3 + 2];
+    double fb = 1.0;                                                               // Ri <= 0
+    if (N2 > 0.0) {
+      double Ri = N2 / (2.0 * ss);                                                 // |S|^2 = 0: Ri = inf, f_b = 0
+      double t = 1.0 - Ri / c.Pr_t;
+      fb = (t > 0.0) ? std::sqrt(std::sqrt(t)) : 0.0;                               // eq. (40)
+    }
+    nu *= fb;
+  }
+  return nu;
 }
 
-void flux_second_order(const Ctx& c, const double* Y, const Prim& P, const double* G, double J, double (*F)[3]) {
-  double nu = eddy_viscosity(c, G, J);
+void flux_second_order(const Ctx& c, const double* Y, const Prim& P, const double* G, double J, const double* dxd,
+                       double (*F)[3]) {
+  double nu = eddy_viscosity(c, G, J, dxd, P.theta_v);
   double Dt = nu / c.Pr_t;                                   // eq. (36)
   double tau[3][3];
   for (int i = 0; i < 3; ++i)
@@ -367,8 +447,46 @@ void flux_second_order(const Ctx& c, const double* Y, const Prim& P, const doubl
   }
 }
 
+// ---------------------------------------------------------------- O8: numerical flux n.F1* of two states
+// riemann = 0: Rusanov (eq. 27 with R1, R2).  riemann = 1: HLLC (named at P:L256; Toro, Spruce & Speares 1994) with the
+// wave-speed estimates S_L = min(u_L - c_L, u_R - c_R), S_R = max(u_L + c_L, u_R + c_R); the momentum flux carries
+// p' = p - p_r (the reference pressure is the same on both sides of a face), the energy flux the full p; rho q is
+// advected with the mass flux.  L = "-" side, R = "+" side, velocities along the outward normal n.
+void numerical_flux(const Ctx& c, const double* Ym, const Prim& Pm, const double (*F1m)[3], const double* Yp, const Prim& Pp,
+                    const double (*F1p)[3], const double* nrm, double* Fstar) {
+  const int nv = c.nvar;
+  double unm = Pm.u[0] * nrm[0] + Pm.u[1] * nrm[1] + Pm.u[2] * nrm[2];
+  double unp = Pp.u[0] * nrm[0] + Pp.u[1] * nrm[1] + Pp.u[2] * nrm[2];
+  double nFm[6], nFp[6];
+  for (int v = 0; v < nv; ++v) {
+    nFm[v] = 0; nFp[v] = 0;
+    for (int cc = 0; cc < 3; ++cc) { nFm[v] += nrm[cc] * F1m[v][cc]; nFp[v] += nrm[cc] * F1p[v][cc]; }
+  }
+  if (c.riemann == 0) {
+    double lam = std::max(std::fabs(unm) + Pm.c, std::fabs(unp) + Pp.c);   // R2
+    for (int v = 0; v < nv; ++v) Fstar[v] = 0.5 * (nFm[v] + nFp[v]) + 0.5 * lam * (Ym[v] - Yp[v]);   // eq. (27), reading R1
+    return;
+  }
+  double SL = std::min(unm - Pm.c, unp - Pp.c), SR = std::max(unm + Pm.c, unp + Pp.c);
+  double Sstar = ((Pp.pp - Pm.pp) + Ym[0] * unm * (SL - unm) - Yp[0] * unp * (SR - unp)) /
+                 (Ym[0] * (SL - unm) - Yp[0] * (SR - unp));
+  if (SL >= 0.0) { for (int v = 0; v < nv; ++v) Fstar[v] = nFm[v]; return; }
+  if (SR <= 0.0) { for (int v = 0; v < nv; ++v) Fstar[v] = nFp[v]; return; }
+  const bool left = Sstar >= 0.0;
+  const double* Y = left ? Ym : Yp; const Prim& P = left ? Pm : Pp;
+  const double un = left ? unm : unp, SK = left ? SL : SR;
+  const double* nF = left ? nFm : nFp;
+  double fac = Y[0] * (SK - un) / (SK - Sstar);            // rho*_K
+  double Us[6];
+  Us[0] = fac;
+  for (int i = 0; i < 3; ++i) Us[1 + i] = fac * (P.u[i] + (Sstar - un) * nrm[i]);
+  Us[4] = fac * (Y[4] / Y[0] + (Sstar - un) * (Sstar + P.p / (Y[0] * (SK - un))));
+  if (nv == 6) Us[5] = fac * P.q;
+  for (int v = 0; v < nv; ++v) Fstar[v] = nF[v] + SK * (Us[v] - Y[v]);
+}
+
 // ---------------------------------------------------------------- O7/O8: tendency of one element
-// Ge = gradient of this element [Np][15]; Gn[f] = gradient array of the neighbour across face f (or null).
+// Ge = gradient of this element [Np][18]; Gn[f] = gradient array of the neighbour across face f (or null).
 // form: 0 weak (eq. 26), 1 strong (eq. 32).
 void rhs_element(const Ctx& c, const double* Q, int64_t e, const double* Ge, const double* const* Gn, int form,
                  double* dQ) {
@@ -382,7 +500,7 @@ void rhs_element(const Ctx& c, const double* Q, int64_t e, const double* Ge, con
     P[n] = prim_at(c, Q, e, n, g.x[3 * n + 2]);
     double F1[6][3], F2[6][3];
     flux_first_order(c, Y, P[n], F1);
-    if (c.sgs) flux_second_order(c, Y, P[n], Ge + 15 * n, g.J[n], F2);
+    if (c.sgs) flux_second_order(c, Y, P[n], Ge + NG3 * n, g.J[n], g.dxd + 3 * n, F2);
     const double* a = g.Ja + 9 * n;
     for (int v = 0; v < nv; ++v) {
       double F[3];
@@ -421,6 +539,14 @@ void rhs_element(const Ctx& c, const double* Q, int64_t e, const double* Ge, con
         }
         // source: -(rho - rho_r) grad Phi, grad Phi = g zhat          (eq. 4)
         dQ[(size_t)n * nv + 3] += -(P[n].rho - P[n].rho_r) * c.grav;
+        // Rayleigh sponge (A4)-(A5) with reading R18 (the pi that (A5) lacks): tau_s = alpha sin^gamma(pi/2 (z-z_s)/(z_top-z_s))
+        double z = g.x[3 * n + 2];
+        if (c.sponge_alpha > 0.0 && z > c.sponge_zs) {
+          const double pi = 3.14159265358979323846;
+          double tau = c.sponge_alpha * std::pow(std::sin(0.5 * pi * (z - c.sponge_zs) / (c.hi[2] - c.sponge_zs)), c.sponge_gamma);
+          const double* Y = Q + ((size_t)e * Np + n) * nv;
+          for (int i = 0; i < 3; ++i) dQ[(size_t)n * nv + 1 + i] -= tau * (Y[1 + i] - Y[0] * c.u_relax[i]);
+        }
       }
   // surface term
   for (int f = 0; f < 6; ++f) {
@@ -438,7 +564,7 @@ void rhs_element(const Ctx& c, const double* Q, int64_t e, const double* Ge, con
         const Prim& Pm = P[n];
         double F1m[6][3]; flux_first_order(c, Ym, Pm, F1m);
         double F2m[6][3];
-        if (c.sgs) flux_second_order(c, Ym, Pm, Ge + 15 * n, g.J[n], F2m);
+        if (c.sgs) flux_second_order(c, Ym, Pm, Ge + NG3 * n, g.J[n], g.dxd + 3 * n, F2m);
         double Yp[6]; Prim Pp; double F1p[6][3], F2p[6][3];
         double Fstar[6];
         if (en >= 0) {
@@ -447,7 +573,7 @@ void rhs_element(const Ctx& c, const double* Q, int64_t e, const double* Ge, con
           for (int v = 0; v < nv; ++v) Yp[v] = Yn[v];
           Pp = prim_at(c, Q, en, nn, gn.x[3 * nn + 2]);
           flux_first_order(c, Yp, Pp, F1p);
-          if (c.sgs) flux_second_order(c, Yp, Pp, Gn[f] + 15 * nn, gn.J[nn], F2p);
+          if (c.sgs) flux_second_order(c, Yp, Pp, Gn[f] + NG3 * nn, gn.J[nn], gn.dxd + 3 * nn, F2p);
         } else {
           // wall ghost state: mirror the normal momentum (A6)-(A7); scalars copied (A8); p_r^+ = p_r^-
           double mn = Ym[1] * nrm[0] + Ym[2] * nrm[1] + Ym[3] * nrm[2];
@@ -457,21 +583,13 @@ void rhs_element(const Ctx& c, const double* Q, int64_t e, const double* Ge, con
           for (int i = 0; i < 3; ++i) Pp.u[i] = Yp[1 + i] / Yp[0];
           flux_first_order(c, Yp, Pp, F1p);
         }
-        double unm = Pm.u[0] * nrm[0] + Pm.u[1] * nrm[1] + Pm.u[2] * nrm[2];
-        double unp = Pp.u[0] * nrm[0] + Pp.u[1] * nrm[1] + Pp.u[2] * nrm[2];
-        double lam = std::max(std::fabs(unm) + Pm.c, std::fabs(unp) + Pp.c);   // R2
-        for (int v = 0; v < nv; ++v) {
-          double nFm = 0, nFp = 0;
-          for (int cc = 0; cc < 3; ++cc) { nFm += nrm[cc] * F1m[v][cc]; nFp += nrm[cc] * F1p[v][cc]; }
-          Fstar[v] = 0.5 * (nFm + nFp) + 0.5 * lam * (Ym[v] - Yp[v]);         // eq. (27), reading R1
-          if (c.sgs) {
-            if (en >= 0) {
-              double a2 = 0;
-              for (int cc = 0; cc < 3; ++cc) a2 += nrm[cc] * 0.5 * (F2m[v][cc] + F2p[v][cc]);   // P:L274, R6
-              Fstar[v] += a2;
-            }  // wall: n.F2* = 0 (R10)
-          }
-        }
+        numerical_flux(c, Ym, Pm, F1m, Yp, Pp, F1p, nrm, Fstar);               // eq. (27) / HLLC
+        if (c.sgs && en >= 0)
+          for (int v = 0; v < nv; ++v) {
+            double a2 = 0;
+            for (int cc = 0; cc < 3; ++cc) a2 += nrm[cc] * 0.5 * (F2m[v][cc] + F2p[v][cc]);   // P:L274, R6
+            Fstar[v] += a2;
+          }  // wall: n.F2* = 0 (R10)
         if (en < 0 && f == 4 && c.shf_bottom != 0.0) Fstar[4] += -c.shf_bottom;  // prescribed upward energy flux
         for (int v = 0; v < nv; ++v) {
           if (form == 0) {
@@ -488,19 +606,19 @@ void rhs_element(const Ctx& c, const double* Q, int64_t e, const double* Ge, con
 
 void gradient_all(const Ctx& c, const double* Q, double* G) {
 #pragma omp parallel for schedule(static)
-  for (int64_t e = 0; e < c.Ne; ++e) gradient_element(c, Q, e, G + (size_t)e * c.Np * 15);
+  for (int64_t e = 0; e < c.Ne; ++e) gradient_element(c, Q, e, G + (size_t)e * c.Np * NG3);
 }
 
 void rhs_all(const Ctx& c, const double* Q, double* dQ, int form) {
   std::vector<double> G;
-  if (c.sgs) { G.resize((size_t)c.Ne * c.Np * 15); gradient_all(c, Q, G.data()); }
+  if (c.sgs) { G.resize((size_t)c.Ne * c.Np * NG3); gradient_all(c, Q, G.data()); }
 #pragma omp parallel for schedule(static)
   for (int64_t e = 0; e < c.Ne; ++e) {
     const double* Gn[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     const double* Ge = nullptr;
     if (c.sgs) {
-      Ge = &G[(size_t)e * c.Np * 15];
-      for (int f = 0; f < 6; ++f) { int64_t en = neighbour(c, e, f); if (en >= 0) Gn[f] = &G[(size_t)en * c.Np * 15]; }
+      Ge = &G[(size_t)e * c.Np * NG3];
+      for (int f = 0; f < 6; ++f) { int64_t en = neighbour(c, e, f); if (en >= 0) Gn[f] = &G[(size_t)en * c.Np * NG3]; }
     }
     rhs_element(c, Q, e, Ge, Gn, form, dQ + (size_t)e * c.Np * c.nvar);
   }
@@ -514,6 +632,82 @@ const double RKB[5] = {1432997174477.0 / 9575080441755.0, 5161836677717.0 / 1361
                        2277821191437.0 / 14882151754819.0};
 const double RKC[5] = {0.0, 1432997174477.0 / 9575080441755.0, 2526269341429.0 / 6820363962896.0,
                        2006345519317.0 / 3224310063776.0, 2802321613138.0 / 2924317926251.0};
+
+
+// ---------------------------------------------------------------- O12: exponential element filter (eq. 52)
+// 1-D nodal filter matrix F = V diag(sigma) V^-1, V_ij = P_j(xi_i) (Legendre modes at the LGL nodes),
+// sigma_j = exp(-alpha (j / N)^s): eta = mode number / polynomial order (R26), s = filter order, alpha = -log(eps_M).
+void filter_matrix(int N, const double* xi, int order, double alpha, double (*F)[MAXNQ]) {
+  const int Nq = N + 1;
+  double V[MAXNQ][MAXNQ], Vi[MAXNQ][MAXNQ];
+  for (int i = 0; i < Nq; ++i)
+    for (int j = 0; j < Nq; ++j) { double P, dP; legendre(j, xi[i], P, dP); V[i][j] = P; }
+  // inverse by Gauss-Jordan with partial pivoting
+  double A[MAXNQ][2 * MAXNQ];
+  for (int i = 0; i < Nq; ++i)
+    for (int j = 0; j < Nq; ++j) { A[i][j] = V[i][j]; A[i][Nq + j] = (i == j) ? 1.0 : 0.0; }
+  for (int col = 0; col < Nq; ++col) {
+    int piv = col;
+    for (int r = col + 1; r < Nq; ++r) if (std::fabs(A[r][col]) > std::fabs(A[piv][col])) piv = r;
+    for (int j = 0; j < 2 * Nq; ++j) std::swap(A[col][j], A[piv][j]);
+    double d = A[col][col];
+    for (int j = 0; j < 2 * Nq; ++j) A[col][j] /= d;
+    for (int r = 0; r < Nq; ++r)
+      if (r != col) { double f = A[r][col]; for (int j = 0; j < 2 * Nq; ++j) A[r][j] -= f * A[col][j]; }
+  }
+  for (int i = 0; i < Nq; ++i) for (int j = 0; j < Nq; ++j) Vi[i][j] = A[i][Nq + j];
+  for (int i = 0; i < Nq; ++i)
+    for (int j = 0; j < Nq; ++j) {
+      double a = 0;
+      for (int m = 0; m < Nq; ++m) a += V[i][m] * std::exp(-alpha * std::pow((double)m / N, order)) * Vi[m][j];
+      F[i][j] = a;
+    }
+}
+
+// Q <- Q_ref + (F x F x F)(Q - Q_ref) on every element and prognostic field: "applied to perturbations of the prognostic
+// variables from the balanced background state"; Q_ref = (rho_r, 0, rhoe_r, rhoq_r), zero without reference.
+void apply_filter(const Ctx& c, double* Q) {
+  const int Nq = c.Nq, Np = c.Np, nv = c.nvar;
+#pragma omp parallel for schedule(static)
+  for (int64_t e = 0; e < c.Ne; ++e) {
+    std::vector<double> a(Np), b(Np), ref(Np);
+    for (int v = 0; v < nv; ++v) {
+      for (int n = 0; n < Np; ++n) {
+        size_t id = (size_t)e * Np + n;
+        ref[n] = 0.0;
+        if (c.use_ref) ref[n] = (v == 0) ? c.ref_rho[id] : (v == 4) ? c.ref_rhoe[id] : (v == 5) ? c.ref_rhoq[id] : 0.0;
+        a[n] = Q[id * nv + v] - ref[n];
+      }
+      for (int k = 0; k < Nq; ++k) for (int j = 0; j < Nq; ++j) for (int i = 0; i < Nq; ++i) {
+        double t = 0; for (int m = 0; m < Nq; ++m) t += c.Filt[i][m] * a[m + Nq * (j + Nq * k)];
+        b[i + Nq * (j + Nq * k)] = t;
+      }
+      for (int k = 0; k < Nq; ++k) for (int j = 0; j < Nq; ++j) for (int i = 0; i < Nq; ++i) {
+        double t = 0; for (int m = 0; m < Nq; ++m) t += c.Filt[j][m] * b[i + Nq * (m + Nq * k)];
+        a[i + Nq * (j + Nq * k)] = t;
+      }
+      for (int k = 0; k < Nq; ++k) for (int j = 0; j < Nq; ++j) for (int i = 0; i < Nq; ++i) {
+        double t = 0; for (int m = 0; m < Nq; ++m) t += c.Filt[k][m] * a[i + Nq * (j + Nq * m)];
+        b[i + Nq * (j + Nq * k)] = t;
+      }
+      for (int n = 0; n < Np; ++n) Q[((size_t)e * Np + n) * nv + v] = ref[n] + b[n];
+    }
+  }
+}
+
+// ---------------------------------------------------------------- O9/O13: 2N-storage Runge-Kutta with any coefficient table
+// for s: dU <- A_s dU + dt RHS(U); U <- U + B_s dU; the element filter, when enabled, follows every step.
+void lsrk_steps(const Ctx& c, double* Q, double dt, int nsteps, int nstages, const double* A, const double* B) {
+  size_t n = (size_t)c.Ne * c.Np * c.nvar;
+  std::vector<double> dU(n, 0.0), R(n);
+  for (int step = 0; step < nsteps; ++step) {
+    for (int s = 0; s < nstages; ++s) {
+      rhs_all(c, Q, R.data(), 0);
+      for (size_t i = 0; i < n; ++i) { dU[i] = A[s] * dU[i] + dt * R[i]; Q[i] = Q[i] + B[s] * dU[i]; }
+    }
+    if (c.filter_order > 0) apply_filter(c, Q);
+  }
+}
 
 }  // namespace
 
@@ -536,6 +730,12 @@ struct odg_params {
   const double *ref_rho, *ref_rhoe, *ref_rhoq;
   double shf_bottom;
   int32_t cache_geometry;
+  int32_t richardson;
+  double p_0;
+  double sponge_alpha, sponge_zs; int32_t sponge_gamma; double u_relax[3];
+  int32_t filter_order; double filter_alpha;
+  int32_t riemann;
+  int32_t metric_form;
 };
 
 void odg_lgl(int N, double* xi, double* w) { lgl_nodes_weights(N, xi, w); }
@@ -560,8 +760,14 @@ void* odg_create(const odg_params* p) {
   c->R_d = p->R_d; c->c_vd = p->c_vd; c->R_v = p->R_v; c->c_vv = p->c_vv; c->T_0 = p->T_0; c->I_v0 = p->I_v0;
   c->grav = p->grav; c->sgs = p->sgs; c->C_s = p->C_s; c->Pr_t = p->Pr_t; c->use_ref = p->use_ref;
   c->shf_bottom = p->shf_bottom;
+  c->richardson = p->richardson; c->p_0 = p->p_0;
+  c->sponge_alpha = p->sponge_alpha; c->sponge_zs = p->sponge_zs; c->sponge_gamma = p->sponge_gamma;
+  for (int d = 0; d < 3; ++d) c->u_relax[d] = p->u_relax[d];
+  c->filter_order = p->filter_order; c->filter_alpha = p->filter_alpha;
+  c->riemann = p->riemann; c->metric_form = p->metric_form;
   lgl_nodes_weights(c->N, c->xi, c->w);
   deriv_matrix(c->N, c->xi, c->D);
+  if (c->filter_order > 0) filter_matrix(c->N, c->xi, c->filter_order, c->filter_alpha, c->Filt);
   size_t nn = (size_t)c->Ne * c->Np;
   if (c->geom == 1) c->zsfc.assign(p->zsfc_nodes, p->zsfc_nodes + (size_t)c->ne[0] * c->Nq * c->ne[1] * c->Nq);
   if (c->geom == 2) c->xyz_in.assign(p->xyz, p->xyz + 3 * nn);
@@ -571,10 +777,11 @@ void* odg_create(const odg_params* p) {
     if (c->nvar == 6) c->ref_rhoq.assign(p->ref_rhoq, p->ref_rhoq + nn);
   }
   if (p->cache_geometry) {
-    c->cx.resize(nn * 3); c->cJa.resize(nn * 9); c->cJ.resize(nn);
+    c->cx.resize(nn * 3); c->cJa.resize(nn * 9); c->cJ.resize(nn); c->cDx.resize(nn * 3);
 #pragma omp parallel for schedule(static)
     for (int64_t e = 0; e < c->Ne; ++e)
-      elem_geo_compute(*c, e, &c->cx[(size_t)e * c->Np * 3], &c->cJa[(size_t)e * c->Np * 9], &c->cJ[(size_t)e * c->Np]);
+      elem_geo_compute(*c, e, &c->cx[(size_t)e * c->Np * 3], &c->cJa[(size_t)e * c->Np * 9], &c->cJ[(size_t)e * c->Np],
+                       &c->cDx[(size_t)e * c->Np * 3]);
     c->cached = true;
   }
   return c;
@@ -615,12 +822,19 @@ void odg_elem_geometry(void* h, int64_t e, double* Ja, double* J, double* M, dou
 
 int64_t odg_neighbour(void* h, int64_t e, int f) { return neighbour(*(Ctx*)h, e, f); }
 
-// pointwise thermodynamics: out = rho,u,v,w,q,T,p,pp,htot,c
+// diagonal of dx/dxi at the nodes of element e: dxd[n][3]
+void odg_elem_dxd(void* h, int64_t e, double* dxd) {
+  const Ctx& c = *(Ctx*)h;
+  Geo g; elem_geo(c, e, g);
+  for (int n = 0; n < 3 * c.Np; ++n) dxd[n] = g.dxd[n];
+}
+
+// pointwise thermodynamics: out = rho,u,v,w,q,T,p,pp,htot,c,theta_v
 void odg_primitives(void* h, const double* Y, double z, int has_ref, double rr, double rer, double rqr, double* out) {
   const Ctx& c = *(Ctx*)h;
   Prim P = primitives(c, Y, z, has_ref != 0, rr, rer, rqr);
   out[0] = P.rho; out[1] = P.u[0]; out[2] = P.u[1]; out[3] = P.u[2]; out[4] = P.q; out[5] = P.T; out[6] = P.p;
-  out[7] = P.pp; out[8] = P.htot; out[9] = P.c;
+  out[7] = P.pp; out[8] = P.htot; out[9] = P.c; out[10] = P.theta_v;
 }
 
 // pointwise Rusanov flux n.F1* of two states at height z without reference state (pins: consistency, symmetry)
@@ -629,14 +843,7 @@ void odg_rusanov(void* h, const double* Ym, const double* Yp, const double* nrm,
   Prim Pm = primitives(c, Ym, z, false, 0, 0, 0), Pp = primitives(c, Yp, z, false, 0, 0, 0);
   double F1m[6][3], F1p[6][3];
   flux_first_order(c, Ym, Pm, F1m); flux_first_order(c, Yp, Pp, F1p);
-  double unm = Pm.u[0] * nrm[0] + Pm.u[1] * nrm[1] + Pm.u[2] * nrm[2];
-  double unp = Pp.u[0] * nrm[0] + Pp.u[1] * nrm[1] + Pp.u[2] * nrm[2];
-  double lam = std::max(std::fabs(unm) + Pm.c, std::fabs(unp) + Pp.c);
-  for (int v = 0; v < c.nvar; ++v) {
-    double nFm = 0, nFp = 0;
-    for (int cc = 0; cc < 3; ++cc) { nFm += nrm[cc] * F1m[v][cc]; nFp += nrm[cc] * F1p[v][cc]; }
-    Fstar[v] = 0.5 * (nFm + nFp) + 0.5 * lam * (Ym[v] - Yp[v]);
-  }
+  numerical_flux(c, Ym, Pm, F1m, Yp, Pp, F1p, nrm, Fstar);   // Rusanov or HLLC, as the ctx says
 }
 
 // physical first-order flux F1[v][3] at a point (no reference state)
@@ -647,17 +854,26 @@ void odg_flux1(void* h, const double* Y, double z, double* F) {
   for (int v = 0; v < c.nvar; ++v) for (int cc = 0; cc < 3; ++cc) F[v * 3 + cc] = F1[v][cc];
 }
 
-// second-order flux F2[v][3] at a point given the gradient G[5][3] and the metric determinant J
-void odg_flux2(void* h, const double* Y, double z, const double* G, double J, double* F, double* nu_t) {
+// second-order flux F2[v][3] at a point given the gradient G[6][3] (u, v, w, h_tot, q, theta_v), the metric
+// determinant J and the diagonal dxd[3] of dx/dxi (mixing lengths of the Vreman model)
+void odg_flux2(void* h, const double* Y, double z, const double* G, double J, const double* dxd, double* F, double* nu_t) {
   const Ctx& c = *(Ctx*)h;
   Prim P = primitives(c, Y, z, false, 0, 0, 0);
-  double F2[6][3]; flux_second_order(c, Y, P, G, J, F2);
+  double F2[6][3]; flux_second_order(c, Y, P, G, J, dxd, F2);
   for (int v = 0; v < c.nvar; ++v) for (int cc = 0; cc < 3; ++cc) F[v * 3 + cc] = F2[v][cc];
-  *nu_t = eddy_viscosity(c, G, J);
+  *nu_t = eddy_viscosity(c, G, J, dxd, P.theta_v);
 }
 
 // BR1 gradient of the whole mesh: G[e][n][5][3]
-void odg_gradient(void* h, const double* Q, double* G) { gradient_all(*(Ctx*)h, Q, G); }
+void odg_gradient(void* h, const double* Q, double* G) {
+  const Ctx& c = *(Ctx*)h;
+  std::vector<double> G6((size_t)c.Ne * c.Np * NG3);
+  gradient_all(c, Q, G6.data());
+  for (size_t i = 0; i < (size_t)c.Ne * c.Np; ++i)
+    for (int m = 0; m < 15; ++m) G[i * 15 + m] = G6[i * NG3 + m];
+}
+// the same with the sixth gradient variable theta_v: G[e][n][6][3]
+void odg_gradient6(void* h, const double* Q, double* G) { gradient_all(*(Ctx*)h, Q, G); }
 
 // dQ[e][n][v] = RHS(Q); form 0 = weak (eq. 26), 1 = strong (eq. 32)
 void odg_rhs(void* h, const double* Q, double* dQ, int form) { rhs_all(*(Ctx*)h, Q, dQ, form); }
@@ -671,10 +887,10 @@ void odg_rhs_elements(void* h, const double* Q, const int64_t* elems, int64_t ne
     std::vector<double> Ge, Gnb[6];
     const double* Gn[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     if (c.sgs) {
-      Ge.resize((size_t)c.Np * 15); gradient_element(c, Q, e, Ge.data());
+      Ge.resize((size_t)c.Np * NG3); gradient_element(c, Q, e, Ge.data());
       for (int f = 0; f < 6; ++f) {
         int64_t en = neighbour(c, e, f);
-        if (en >= 0) { Gnb[f].resize((size_t)c.Np * 15); gradient_element(c, Q, en, Gnb[f].data()); Gn[f] = Gnb[f].data(); }
+        if (en >= 0) { Gnb[f].resize((size_t)c.Np * NG3); gradient_element(c, Q, en, Gnb[f].data()); Gn[f] = Gnb[f].data(); }
       }
     }
     rhs_element(c, Q, e, c.sgs ? Ge.data() : nullptr, Gn, 0, out + (size_t)s * c.Np * c.nvar);
@@ -683,15 +899,21 @@ void odg_rhs_elements(void* h, const double* Q, const int64_t* elems, int64_t ne
 
 // LSRK54: for s: dU <- A_s dU + dt RHS(U, t + C_s dt); U <- U + B_s dU
 void odg_lsrk54(void* h, double* Q, double t, double dt, int nsteps) {
-  const Ctx& c = *(Ctx*)h;
   (void)t;
-  size_t n = (size_t)c.Ne * c.Np * c.nvar;
-  std::vector<double> dU(n, 0.0), R(n);
-  for (int step = 0; step < nsteps; ++step)
-    for (int s = 0; s < 5; ++s) {
-      rhs_all(c, Q, R.data(), 0);
-      for (size_t i = 0; i < n; ++i) { dU[i] = RKA[s] * dU[i] + dt * R[i]; Q[i] = Q[i] + RKB[s] * dU[i]; }
-    }
+  lsrk_steps(*(Ctx*)h, Q, dt, nsteps, 5, RKA, RKB);
+}
+
+// the same for any 2N-storage coefficient table (A_1 must be 0), e.g. the 14-stage scheme the paper ran
+void odg_lsrk_table(void* h, double* Q, double dt, int nsteps, int nstages, const double* A, const double* B) {
+  lsrk_steps(*(Ctx*)h, Q, dt, nsteps, nstages, A, B);
+}
+
+// exponential element filter (eq. 52) applied once, in place; the 1-D filter matrix [Nq][Nq] row-major
+void odg_filter(void* h, double* Q) { apply_filter(*(Ctx*)h, Q); }
+void odg_filter_matrix(int N, int order, double alpha, double* Fout) {
+  double xi[MAXNQ], w[MAXNQ], F[MAXNQ][MAXNQ];
+  lgl_nodes_weights(N, xi, w); filter_matrix(N, xi, order, alpha, F);
+  for (int i = 0; i <= N; ++i) for (int j = 0; j <= N; ++j) Fout[i * (N + 1) + j] = F[i][j];
 }
 
 // forward Euler: U <- U + dt RHS(U)

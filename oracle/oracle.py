@@ -36,6 +36,9 @@ class _Params(C.Structure):
         ("sgs", C.c_int32), ("C_s", C.c_double), ("Pr_t", C.c_double), ("use_ref", C.c_int32),
         ("ref_rho", C.POINTER(C.c_double)), ("ref_rhoe", C.POINTER(C.c_double)), ("ref_rhoq", C.POINTER(C.c_double)),
         ("shf_bottom", C.c_double), ("cache_geometry", C.c_int32),
+        ("richardson", C.c_int32), ("p_0", C.c_double),
+        ("sponge_alpha", C.c_double), ("sponge_zs", C.c_double), ("sponge_gamma", C.c_int32), ("u_relax", C.c_double * 3),
+        ("filter_order", C.c_int32), ("filter_alpha", C.c_double), ("riemann", C.c_int32), ("metric_form", C.c_int32),
     ]
 
 
@@ -67,8 +70,13 @@ def lib():
             "odg_primitives": [C.c_void_p, _dp, C.c_double, C.c_int, C.c_double, C.c_double, C.c_double, _dp],
             "odg_rusanov": [C.c_void_p, _dp, _dp, _dp, C.c_double, _dp],
             "odg_flux1": [C.c_void_p, _dp, C.c_double, _dp],
-            "odg_flux2": [C.c_void_p, _dp, C.c_double, _dp, C.c_double, _dp, _dp],
+            "odg_flux2": [C.c_void_p, _dp, C.c_double, _dp, C.c_double, _dp, _dp, _dp],
             "odg_gradient": [C.c_void_p, _dp, _dp],
+            "odg_gradient6": [C.c_void_p, _dp, _dp],
+            "odg_elem_dxd": [C.c_void_p, C.c_int64, _dp],
+            "odg_lsrk_table": [C.c_void_p, _dp, C.c_double, C.c_int, C.c_int, _dp, _dp],
+            "odg_filter": [C.c_void_p, _dp],
+            "odg_filter_matrix": [C.c_int, C.c_int, C.c_double, _dp],
             "odg_rhs": [C.c_void_p, _dp, _dp, C.c_int],
             "odg_rhs_elements": [C.c_void_p, _dp, C.POINTER(C.c_int64), C.c_int64, _dp],
             "odg_lsrk54": [C.c_void_p, _dp, C.c_double, C.c_double, C.c_int],
@@ -98,6 +106,12 @@ def lsrk54_coeffs():
     A = np.zeros(5); B = np.zeros(5); Cc = np.zeros(5)
     lib().odg_lsrk54_coeffs(_ptr(A), _ptr(B), _ptr(Cc))
     return A, B, Cc
+
+
+def filter_matrix(N, order, alpha=36.0436533891172):
+    F = np.zeros((N + 1, N + 1))
+    lib().odg_filter_matrix(N, int(order), float(alpha), _ptr(F))
+    return F
 
 
 def num_threads():
@@ -144,6 +158,14 @@ class Oracle:
                 assert a.size == self.Ne * self.Np
                 self._keep.append(a); setattr(p, k, _ptr(a))
         p.cache_geometry = 1 if cache_geometry else 0
+        # optional physics / numerics beyond the five BASELINE configs (defaults = off)
+        p.richardson = int(cfg.get("richardson", 0))
+        p.p_0 = float(cfg.get("p_0", 1.0e5))
+        p.sponge_alpha = float(cfg.get("sponge_alpha", 0.0)); p.sponge_zs = float(cfg.get("sponge_zs", 0.0))
+        p.sponge_gamma = int(cfg.get("sponge_gamma", 2))
+        p.u_relax[:] = [float(v) for v in cfg.get("u_relax", (0.0, 0.0, 0.0))]
+        p.filter_order = int(cfg.get("filter_order", 0)); p.filter_alpha = float(cfg.get("filter_alpha", 36.0436533891172))
+        p.riemann = int(cfg.get("riemann", 0)); p.metric_form = int(cfg.get("metric_form", 0))
         self._h = L.odg_create(C.byref(p))
         if not self._h:
             raise ValueError("odg_create rejected the parameters")
@@ -182,12 +204,12 @@ class Oracle:
 
     # ---- pointwise
     def primitives(self, Y, z=0.0, ref=None):
-        Y = np.ascontiguousarray(Y, dtype=np.float64); out = np.zeros(10)
+        Y = np.ascontiguousarray(Y, dtype=np.float64); out = np.zeros(11)
         if ref is None:
             lib().odg_primitives(self._h, _ptr(Y), float(z), 0, 0.0, 0.0, 0.0, _ptr(out))
         else:
             lib().odg_primitives(self._h, _ptr(Y), float(z), 1, float(ref[0]), float(ref[1]), float(ref[2]), _ptr(out))
-        return dict(zip(("rho", "u", "v", "w", "q", "T", "p", "pp", "htot", "c"), out))
+        return dict(zip(("rho", "u", "v", "w", "q", "T", "p", "pp", "htot", "c", "theta_v"), out))
 
     def rusanov(self, Ym, Yp, n, z=0.0):
         Ym = np.ascontiguousarray(Ym, dtype=np.float64); Yp = np.ascontiguousarray(Yp, dtype=np.float64)
@@ -200,11 +222,19 @@ class Oracle:
         lib().odg_flux1(self._h, _ptr(Y), float(z), _ptr(F))
         return F
 
-    def flux2(self, Y, G, J, z=0.0):
-        Y = np.ascontiguousarray(Y, dtype=np.float64); G = np.ascontiguousarray(G, dtype=np.float64)
+    def flux2(self, Y, G, J, z=0.0, dxd=None):
+        """G: [5][3] (u, v, w, h_tot, q) or [6][3] with theta_v; dxd: diagonal of dx/dxi (default: a cube of volume 8 J)."""
+        Y = np.ascontiguousarray(Y, dtype=np.float64)
+        G6 = np.zeros((6, 3)); G = np.asarray(G, dtype=np.float64); G6[: G.shape[0]] = G
+        dxd = np.ascontiguousarray(np.full(3, np.cbrt(J)) if dxd is None else dxd, dtype=np.float64)
         F = np.zeros((self.nvar, 3)); nu = np.zeros(1)
-        lib().odg_flux2(self._h, _ptr(Y), float(z), _ptr(G), float(J), _ptr(F), _ptr(nu))
+        lib().odg_flux2(self._h, _ptr(Y), float(z), _ptr(G6), float(J), _ptr(dxd), _ptr(F), _ptr(nu))
         return F, float(nu[0])
+
+    def elem_dxd(self, e):
+        d = np.zeros((self.Np, 3))
+        lib().odg_elem_dxd(self._h, e, _ptr(d))
+        return d
 
     # ---- operators
     def _q(self, Q):
@@ -215,6 +245,11 @@ class Oracle:
     def gradient(self, Q):
         Q = self._q(Q); G = np.zeros((self.Ne, self.Np, 5, 3))
         lib().odg_gradient(self._h, _ptr(Q), _ptr(G))
+        return G
+
+    def gradient6(self, Q):
+        Q = self._q(Q); G = np.zeros((self.Ne, self.Np, 6, 3))
+        lib().odg_gradient6(self._h, _ptr(Q), _ptr(G))
         return G
 
     def rhs(self, Q, form="weak"):
@@ -231,6 +266,18 @@ class Oracle:
     def lsrk54(self, Q, dt, nsteps, t=0.0):
         Q = self._q(Q).copy()
         lib().odg_lsrk54(self._h, _ptr(Q), float(t), float(dt), int(nsteps))
+        return Q
+
+    def lsrk_table(self, Q, dt, nsteps, A, B):
+        """nsteps steps of the 2N-storage scheme with coefficient tables A, B (A[0] = 0)."""
+        Q = self._q(Q).copy()
+        A = np.ascontiguousarray(A, dtype=np.float64); B = np.ascontiguousarray(B, dtype=np.float64)
+        lib().odg_lsrk_table(self._h, _ptr(Q), float(dt), int(nsteps), int(A.size), _ptr(A), _ptr(B))
+        return Q
+
+    def filter(self, Q):
+        Q = self._q(Q).copy()
+        lib().odg_filter(self._h, _ptr(Q))
         return Q
 
     def euler(self, Q, dt, nsteps):
