@@ -56,12 +56,26 @@ typedef struct {
   const double* zsfc_nodes; /* geom==1: HOST [Ey*Nq][Ex*Nq] surface height at the bottom nodes              */
   const double* xyz;        /* geom==2: HOST [3][Ne][Np], LEXICOGRAPHIC element order                       */
   double R_d, c_vd, R_v, c_vv, T_0, I_v0, grav; /* Table 1, eq. (9); Phi = grav * z     */
-  int32_t sgs;              /* 0 inviscid | 1 Smagorinsky-Lilly (eq. 38)                                    */
+  int32_t sgs;              /* 0 inviscid | 1 Smagorinsky-Lilly (eq. 38) | 2 Vreman (eq. 39a-d)   */
   double C_s, Pr_t;         /* Smagorinsky coefficient, turbulent Prandtl number (eq. 36)                   */
   int32_t use_ref;          /* 1: remove the hydrostatic reference state in the momentum equation (eq. 4)   */
   const double *ref_rho, *ref_rhoe, *ref_rhoq; /* HOST [Ne][Np] LEXICOGRAPHIC; resting reference state;
                                                   p_r is derived from them with the library's EOS          */
   double shf_bottom;        /* W m^-2 prescribed upward energy flux through the z-low wall, 0 = none */
+  /* ---- optional physics and numerics beyond the five BASELINE configs; all-zero = off / defaults ---- */
+  int32_t richardson;       /* 1: multiply nu_t by the stability factor f_b of eq. (40); needs sgs != 0 */
+  double p_0;               /* reference pressure of theta_v in eq. (40) [Pa]; 0 = 1e5                       */
+  double sponge_alpha;      /* Rayleigh sponge (A4)-(A5): relaxation coefficient [1/s], 0 = no sponge */
+  double sponge_zs;         /* height where the absorbing layer starts [m]; it ends at hi[2]                  */
+  int32_t sponge_gamma;     /* power of the sine profile (positive, typically 2); 0 = 2                       */
+  double u_relax[3];        /* velocity the momentum is relaxed to inside the layer [m/s]                     */
+  int32_t filter_order;     /* exponential element filter of eq. (52): order s (even, e.g. 64), 0 = off;
+                               when on, cm_dg_lsrk_step* apply it after every time step (cm_dg_filter applies it once) */
+  double filter_alpha;      /* alpha = -log(eps_M) of eq. (52); 0 = 36.0436533891172 (double precision)       */
+  int32_t riemann;          /* numerical flux of F1: 0 Rusanov (eq. 27) | 1 HLLC; HLLC runs on the
+                               stored-metric kernels                                                          */
+  int32_t metric_form;      /* 0 cross-product metric terms (extruded / 2.5-D warps) | 1 curl-invariant form
+                               (fully 3-D warps; geom == 2)                                                   */
 } cm_dg_params;
 
 /* Optional scheduling knobs (HOST, copied by cm_dg_setup_tuned).  They never change what is computed (the parity tests
@@ -129,6 +143,17 @@ int cm_dg_rhs(cm_dg_ctx* ctx, const double* Q_dev, double* dQ_dev, double t);
  * tendency + low-storage update kernel.  The result is left in Q_dev: the five stages of a step cycle through two
  * ctx-owned buffers and end in the caller's array (no stage updates in place, no copy is appended). */
 int cm_dg_lsrk_step(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t nsteps);
+
+/* The same for any 2N-storage Runge-Kutta scheme given by its coefficient tables (HOST, nstages entries each; A[0]
+ * must be 0): for s: dU <- A_s dU + dt RHS(U, t + C_s dt); U <- U + B_s dU.  cm_dg_lsrk_step is this call
+ * with the Carpenter-Kennedy (5,4) table; the 14-stage scheme the paper ran is a table of 14.  C may be NULL
+ * (no time-dependent forcing on this path).  CM_DG_EINVAL for nstages < 1 or A[0] != 0. */
+int cm_dg_lsrk_step_table(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t nsteps, int32_t nstages,
+                          const double* A, const double* B, const double* C);
+
+/* Exponential element filter of eq. (52) applied once, in place: Q <- Q_ref + (F x F x F)(Q - Q_ref) on every element and
+ * prognostic field, F = V diag(exp(-alpha (n/N)^s)) V^-1 in the Legendre basis.  CM_DG_ESTATE if filter_order == 0. */
+int cm_dg_filter(cm_dg_ctx* ctx, double* Q_dev);
 
 /* a6: conservation integrals etc. of Q_dev into *out_host; synchronises the stream. */
 int cm_dg_diagnostics(cm_dg_ctx* ctx, const double* Q_dev, cm_dg_diag* out_host);

@@ -23,6 +23,9 @@ class _Params(C.Structure):
         ("sgs", C.c_int32), ("C_s", C.c_double), ("Pr_t", C.c_double), ("use_ref", C.c_int32),
         ("ref_rho", C.c_void_p), ("ref_rhoe", C.c_void_p), ("ref_rhoq", C.c_void_p),
         ("shf_bottom", C.c_double),
+        ("richardson", C.c_int32), ("p_0", C.c_double),
+        ("sponge_alpha", C.c_double), ("sponge_zs", C.c_double), ("sponge_gamma", C.c_int32), ("u_relax", C.c_double * 3),
+        ("filter_order", C.c_int32), ("filter_alpha", C.c_double), ("riemann", C.c_int32), ("metric_form", C.c_int32),
     ]
 
 
@@ -43,7 +46,7 @@ class _KStats(C.Structure):
 
 
 EXPORTS = ("cm_dg_setup", "cm_dg_setup_tuned", "cm_dg_layout", "cm_dg_coords", "cm_dg_metrics", "cm_dg_gradient", "cm_dg_rhs",
-           "cm_dg_lsrk_step", "cm_dg_diagnostics", "cm_dg_rhs_host", "cm_dg_lsrk_step_host",
+           "cm_dg_lsrk_step", "cm_dg_lsrk_step_table", "cm_dg_filter", "cm_dg_diagnostics", "cm_dg_rhs_host", "cm_dg_lsrk_step_host",
            "cm_dg_profile_begin", "cm_dg_profile_end", "cm_dg_destroy", "cm_dg_last_error")
 
 _lib = None
@@ -70,6 +73,8 @@ def _load():
     L.cm_dg_gradient.argtypes = [vp, vp, vp]
     L.cm_dg_rhs.argtypes = [vp, vp, vp, dbl]
     L.cm_dg_lsrk_step.argtypes = [vp, vp, dbl, dbl, i32]
+    L.cm_dg_lsrk_step_table.argtypes = [vp, vp, dbl, dbl, i32, i32, vp, vp, vp]
+    L.cm_dg_filter.argtypes = [vp, vp]
     L.cm_dg_diagnostics.argtypes = [vp, vp, C.POINTER(_Diag)]
     L.cm_dg_rhs_host.argtypes = [vp, vp, vp, dbl]
     L.cm_dg_lsrk_step_host.argtypes = [vp, vp, dbl, dbl, i32]
@@ -140,6 +145,11 @@ def cm_dg_setup(cfg, stream=None, tuning=None):
     for k in ("R_d", "c_vd", "R_v", "c_vv", "T_0", "I_v0", "grav", "C_s", "Pr_t", "shf_bottom"):
         setattr(p, k, float(cfg[k]))
     p.sgs = int(cfg.get("sgs", 0))
+    for k in ("richardson", "sponge_gamma", "filter_order", "riemann", "metric_form"):
+        setattr(p, k, int(cfg.get(k, 0)))
+    for k in ("p_0", "sponge_alpha", "sponge_zs", "filter_alpha"):
+        setattr(p, k, float(cfg.get(k, 0.0)))
+    p.u_relax[:] = [float(v) for v in cfg.get("u_relax", (0.0, 0.0, 0.0))]
     p.use_ref = int(cfg.get("use_ref", 0))
     if p.use_ref:
         p.ref_rho = host("ref_rho"); p.ref_rhoe = host("ref_rhoe"); p.ref_rhoq = host("ref_rhoq")
@@ -184,6 +194,18 @@ def cm_dg_rhs(ctx, Q_dev, dQ_dev, t=0.0):
 
 def cm_dg_lsrk_step(ctx, Q_dev, t, dt, nsteps):
     _check(_load().cm_dg_lsrk_step(ctx, _dptr(Q_dev), float(t), float(dt), int(nsteps)), "cm_dg_lsrk_step")
+
+
+def cm_dg_lsrk_step_table(ctx, Q_dev, t, dt, nsteps, A, B, Cc=None):
+    A = np.ascontiguousarray(A, dtype=np.float64); B = np.ascontiguousarray(B, dtype=np.float64)
+    assert A.size == B.size
+    cp = C.c_void_p(np.ascontiguousarray(Cc, dtype=np.float64).ctypes.data) if Cc is not None else C.c_void_p(0)
+    _check(_load().cm_dg_lsrk_step_table(ctx, _dptr(Q_dev), float(t), float(dt), int(nsteps), int(A.size),
+                                         C.c_void_p(A.ctypes.data), C.c_void_p(B.ctypes.data), cp), "cm_dg_lsrk_step_table")
+
+
+def cm_dg_filter(ctx, Q_dev):
+    _check(_load().cm_dg_filter(ctx, _dptr(Q_dev)), "cm_dg_filter")
 
 
 def cm_dg_diagnostics(ctx, Q_dev):
@@ -279,6 +301,14 @@ class CmDg:
 
     def lsrk_step(self, Q, dt, nsteps=1, t=0.0):
         cm_dg_lsrk_step(self.ctx, Q, t, dt, nsteps)
+        return Q
+
+    def lsrk_step_table(self, Q, dt, nsteps, A, B, t=0.0):
+        cm_dg_lsrk_step_table(self.ctx, Q, t, dt, nsteps, A, B)
+        return Q
+
+    def filter(self, Q):
+        cm_dg_filter(self.ctx, Q)
         return Q
 
     def diagnostics(self, Q):

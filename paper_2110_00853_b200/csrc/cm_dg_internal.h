@@ -5,8 +5,8 @@
 #include <cuda_runtime.h>
 
 #define CM_MAXNQ 8
-#define CM_ZTAB_W 8   // doubles per z-table row (flat meshes): Phi, rho_r, rhoe_r, rhoq_r, E_r, q_r, 1/c_vm_r, unused
-#define CM_NGEO 12    // general geometry, per node: Ja[9], 1/J, z, (C_s Delta)^2
+#define CM_ZTAB_W 8   // doubles per z-table row (flat meshes): Phi, rho_r, rhoe_r, rhoq_r, E_r, q_r, 1/c_vm_r, tau_s (sponge)
+#define CM_NGEO 16    // general geometry, per node: Ja[9], 1/J, z, (C_s Delta)^2, Delta_m^2 [3], tau_s (sponge)
 
 // Thermodynamic constants of eq. (7)-(14) in the combinations the kernels use.
 struct CmThermo {
@@ -16,6 +16,7 @@ struct CmThermo {
   double T_0, I_v0, grav;
   double dk;   // a c_vd - R_d b   (numerator of kappa - kappa_r, reading R12)
   double icvd, kappa_d;  // 1 / c_vd, R_d / c_vd (dry air)
+  double p_0, kap_pd, iRd;   // theta_v = (p / (rho R_d)) (p_0 / p)^(R_d / c_pd)   (eq. 40, reading R25)
 };
 
 // Kernel argument block (passed by value, lives in the constant bank).
@@ -29,7 +30,9 @@ struct CmKP {
   int ahead;             // flat: L2 prefetch distance in elements of the launch order (0 = off)
   float ginvL, ginvNXC;  // 1 / gL, 1 / gNXC (exact small-integer division in cm7_position)
   long long stride;      // field stride in doubles
-  int sgs;               // Smagorinsky-Lilly on/off
+  int sgs;               // 0 inviscid | 1 Smagorinsky-Lilly | 2 Vreman
+  int richardson;        // eq. (40): nu_t *= f_b (one more gradient variable, theta_v)
+  int riemann;           // 0 Rusanov | 1 HLLC (stored-metric kernels)
   int use_ref;           // reference state removed (R12) or plain pressure
   int mode;              // tendency: 0 dQ := rhs | 1 LSRK stage.  gradient: 0 packed SGS fluxes | 1 raw 15 gradients
   // arrays
@@ -48,6 +51,9 @@ struct CmKP {
   double cA[3];          // flat: Ja^d_d = h_e h_f / 4
   double invJ;           // flat: 8 / (hx hy hz)
   double cs2delta2;      // flat: (C_s Delta)^2
+  double cs2;            // C_s^2
+  double d2[3];          // flat: squared mixing lengths Delta_m^2 = (h_m / N)^2 of the Vreman model (eq. 39c)
+  double urelax[3];      // Rayleigh sponge: relaxation velocity (eq. A4); tau_s comes with the z table / geometry
   double inv_Pr;
   double shf;            // prescribed upward energy flux at the bottom wall
   double inv_w0;         // 1 / w_0 = N (N+1) / 2

@@ -299,7 +299,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS + 32, CmCfg10<Nq, M
   if (node) {
     const double2* zr = reinterpret_cast<const double2*>(p.ztab + (size_t)(row.pos.ez * Nq + k_) * CM_ZTAB_W);
     const double2 a = __ldg(zr), b = __ldg(zr + 1), c = __ldg(zr + 2), d = __ldg(zr + 3);
-    st.Phi = a.x; st.rho_r = a.y; st.rhoe_r = b.x; st.rhoq_r = b.y; st.E_r = c.x; st.q_r = c.y; st.icvm_r = d.x;
+    st.Phi = a.x; st.rho_r = a.y; st.rhoe_r = b.x; st.rhoq_r = b.y; st.E_r = c.x; st.q_r = c.y; st.icvm_r = d.x; st.taus = d.y;
   }
 
   for (int it = 0; it < S; ++it) {
@@ -418,6 +418,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS + 32, CmCfg10<Nq, M
       for (int v = 0; v < NV; ++v) {
         double rhs = -p.invJ * (acc[v] - p.inv_w0 * lift[v]);
         if (v == 3) rhs -= buoy;                                   // -(rho - rho_r) grad Phi   (eq. 4)
+        if (v >= 1 && v <= 3) rhs -= st.taus * (Y[v] - Y[0] * p.urelax[v - 1]);   // Rayleigh sponge (A4); tau_s = 0 outside the layer
         if (MODE == 0) {
           __stcs(o1, rhs);
         } else {

@@ -37,12 +37,14 @@ __device__ __forceinline__ void cm2_face_nodes(int f, int a, int b, int& nm, int
 // ------------------------------------------------------------------------------------------------
 // a2: auxiliary gradient + Smagorinsky-Lilly, thread per node
 // ------------------------------------------------------------------------------------------------
-template <int Nq, bool MOIST, int GEOM>
+// RICH: theta_v is a further gradient variable (eq. 40)
+template <int Nq, bool MOIST, int GEOM, bool RICH = false>
 __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_gradient_kernel(const __grid_constant__ CmKP p) {
   using C = CmCfg2<Nq>;
   constexpr int NF = C::NF, NP = C::NP, N = Nq - 1, TPE = C::TPE, EPB = C::EPB;
   constexpr int NV = MOIST ? 6 : 5;
-  constexpr int NS = MOIST ? 5 : 4;
+  constexpr int NS0 = MOIST ? 5 : 4;                   // u, v, w, h_tot, [q_t]
+  constexpr int NS = NS0 + (RICH ? 1 : 0);             // + theta_v
   extern __shared__ double smem[];
   double* s_sh = smem;                               // [EPB][NS][NP]      gradient variables
   double* d_sh = s_sh + EPB * NS * NP;               // [3][EPB][NS][NP]   reference-space derivatives
@@ -62,6 +64,7 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_gra
     double* s = s_sh + (size_t)el * NS * NP + t;
     s[0] = P.u; s[NP] = P.v; s[2 * NP] = P.w; s[3 * NP] = P.h;
     if (MOIST) s[4 * NP] = P.q;
+    if (RICH) s[NS0 * NP] = cm_theta_v(p.th, P.p, P.ir);
   }
   __syncthreads();
 
@@ -95,10 +98,9 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_gra
       const int d = f >> 1;
       const double sgn = (f & 1) ? 1.0 : -1.0;
       const int nb = __ldg(p.nbr + (size_t)e * 6 + f);
-      double sm[5], delta[5];
+      double sm[6], delta[6];
 #pragma unroll
       for (int v = 0; v < NS; ++v) sm[v] = s_sh[((size_t)el * NS + v) * NP + nm];
-      if (!MOIST) sm[4] = 0.0;
       if (nb >= e0 && nb < e0 + EPB) {
         const double* sp = s_sh + (size_t)(nb - e0) * NS * NP + np_;
 #pragma unroll
@@ -109,12 +111,14 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_gra
         cm_load_site<Nq, MOIST, GEOM>(p, nb, np_, kp, st);
         cm_eos<MOIST>(p, Y, st, P);
         delta[0] = 0.5 * (P.u - sm[0]); delta[1] = 0.5 * (P.v - sm[1]); delta[2] = 0.5 * (P.w - sm[2]);
-        delta[3] = 0.5 * (P.h - sm[3]); delta[4] = MOIST ? 0.5 * (P.q - sm[4]) : 0.0;
+        delta[3] = 0.5 * (P.h - sm[3]);
+        if (MOIST) delta[4] = 0.5 * (P.q - sm[4]);
+        if (RICH) delta[NS0] = 0.5 * (cm_theta_v(p.th, P.p, P.ir) - sm[NS0]);
       } else {
         // wall: u_bc = u^- - (n.u^-) n  (A6); scalars unchanged (A8)
         double A[3]; cm_face_vector<Nq, GEOM>(p, e, nm, d, sgn, A);
         const double ua = (sm[0] * A[0] + sm[1] * A[1] + sm[2] * A[2]) / (A[0] * A[0] + A[1] * A[1] + A[2] * A[2]);
-        delta[0] = -ua * A[0]; delta[1] = -ua * A[1]; delta[2] = -ua * A[2]; delta[3] = 0.0; delta[4] = 0.0;
+        delta[0] = -ua * A[0]; delta[1] = -ua * A[1]; delta[2] = -ua * A[2]; delta[3] = 0.0; delta[4] = 0.0; delta[5] = 0.0;
       }
       double* fb = fbuf + ((size_t)el * 6 * NF + ft) * NS;
 #pragma unroll
@@ -126,9 +130,9 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_gra
 
   const int n = t, i = n % Nq, j = (n / Nq) % Nq, k = n / NF;
   const size_t idx = (size_t)e * NP + n;
-  double Ja[3][3], invJ, cs2d2;
+  double Ja[3][3], invJ, cs2d2, d2x, d2y, d2z;
   if constexpr (GEOM == 0) {
-    invJ = p.invJ; cs2d2 = p.cs2delta2;
+    invJ = p.invJ; cs2d2 = p.cs2delta2; d2x = p.d2[0]; d2y = p.d2[1]; d2z = p.d2[2];
   } else {
 #pragma unroll
     for (int d = 0; d < 3; ++d)
@@ -136,10 +140,11 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_gra
       for (int c = 0; c < 3; ++c) Ja[d][c] = __ldg(p.geo + (size_t)(3 * d + c) * p.stride + idx);
     invJ = __ldg(p.geo + 9 * p.stride + idx);
     cs2d2 = __ldg(p.geo + 11 * p.stride + idx);
+    d2x = __ldg(p.geo + 12 * p.stride + idx); d2y = __ldg(p.geo + 13 * p.stride + idx); d2z = __ldg(p.geo + 14 * p.stride + idx);
   }
   const double* fb = fbuf + (size_t)el * 6 * NF * NS;
   const double w0i = p.inv_w0;
-  double G[5][3];
+  double G[6][3];
 #pragma unroll
   for (int v = 0; v < NS; ++v) {
     double dr = d_sh[(((size_t)0 * EPB + el) * NS + v) * NP + n];
@@ -158,24 +163,26 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_gra
       for (int c = 0; c < 3; ++c) G[v][c] = invJ * (Ja[0][c] * dr + Ja[1][c] * ds + Ja[2][c] * dt);
     }
   }
-  if (!MOIST) { G[4][0] = G[4][1] = G[4][2] = 0.0; }
+  if (!MOIST) { if (RICH) { G[5][2] = G[4][2]; } G[4][0] = G[4][1] = G[4][2] = 0.0; }   // dry: theta_v sits in slot 4
   if (p.mode == 1) {
 #pragma unroll
     for (int v = 0; v < 5; ++v)
 #pragma unroll
       for (int c = 0; c < 3; ++c) p.Gout[(size_t)(3 * v + c) * p.stride + idx] = G[v][c];
   } else {
-    // eq. (33)-(38): S, nu_t = (C_s Delta)^2 sqrt(2 S:S), D_t = nu_t / Pr_t; store tau, J + D, d_q
-    const double Sxx = G[0][0], Syy = G[1][1], Szz = G[2][2];
-    const double Sxy = 0.5 * (G[0][1] + G[1][0]), Sxz = 0.5 * (G[0][2] + G[2][0]), Syz = 0.5 * (G[1][2] + G[2][1]);
-    const double ss = Sxx * Sxx + Syy * Syy + Szz * Szz + 2.0 * (Sxy * Sxy + Sxz * Sxz + Syz * Syz);
-    const double nu = cs2d2 * cm_sqrt(2.0 * ss);
-    const double m2nu = -2.0 * nu, mDt = -nu * p.inv_Pr;
+    // eq. (33)-(40): closure (cm_closure); store tau, J + D, d_q
+    double Gr[5][3];
+#pragma unroll
+    for (int v = 0; v < 5; ++v)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) Gr[v][c] = G[v][c];
+    double thv = 1.0, dthv = 0.0;
+    if (RICH) { thv = s_sh[((size_t)el * NS + NS0) * NP + n]; dthv = G[5][2]; }
+    double g[12];
+    cm_closure<MOIST>(p, Gr, cs2d2, d2x, d2y, d2z, thv, dthv, g);
     double* o = p.Gout + idx;
-    o[0] = m2nu * Sxx; o[p.stride] = m2nu * Syy; o[2 * p.stride] = m2nu * Szz;
-    o[3 * p.stride] = m2nu * Sxy; o[4 * p.stride] = m2nu * Sxz; o[5 * p.stride] = m2nu * Syz;
-    o[6 * p.stride] = mDt * G[3][0]; o[7 * p.stride] = mDt * G[3][1]; o[8 * p.stride] = mDt * G[3][2];
-    if (MOIST) { o[9 * p.stride] = mDt * G[4][0]; o[10 * p.stride] = mDt * G[4][1]; o[11 * p.stride] = mDt * G[4][2]; }
+#pragma unroll
+    for (int kk = 0; kk < (MOIST ? 12 : 9); ++kk) o[kk * p.stride] = g[kk];
   }
 }
 
@@ -199,7 +206,7 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_ten
   const int e0 = blockIdx.x * EPB;
   const int e = e0 + el;
   const bool active = e < p.Ne;
-  double buoy = 0.0;
+  double buoy = 0.0, taus = 0.0;
 
   // ---- phase 0: primitives and fluxes of the own node -> shared memory
   if (active && t < NP) {
@@ -209,7 +216,7 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_ten
     if (p.sgs) cm_load_state<NG>(p.G, p.stride, idx, g);
     cm_load_site<Nq, MOIST, GEOM>(p, e, t, t / NF, st);
     cm_eos<MOIST>(p, Y, st, P);
-    buoy = P.drho * p.th.grav;
+    buoy = P.drho * p.th.grav; taus = st.taus;
     double* q = Q_sh + (size_t)el * NV * NP + t;
 #pragma unroll
     for (int v = 0; v < NV; ++v) q[v * NP] = Y[v];
@@ -287,9 +294,20 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_ten
           c2p = P.c2;
           uAp = A[0] * P.u + A[1] * P.v + A[2] * P.w;
         }
-        const double lamsJ = fmax(fabs(uAm) + cm_ * sJ, fabs(uAp) + cm_sqrt(c2p) * sJ);   // sJ * lambda (R2)
+        if (p.riemann == 0) {
+          const double lamsJ = fmax(fabs(uAm) + cm_ * sJ, fabs(uAp) + cm_sqrt(c2p) * sJ);   // sJ * lambda (R2)
 #pragma unroll
-        for (int v = 0; v < NV; ++v) r[v] = 0.5 * (Ftm[v] - Fp[v]) - 0.5 * lamsJ * (Ym[v] - Yp[v]);
+          for (int v = 0; v < NV; ++v) r[v] = 0.5 * (Ftm[v] - Fp[v]) - 0.5 * lamsJ * (Ym[v] - Yp[v]);
+        } else {
+          // HLLC for F1, central flux for F2: sJ F* = Fs + (1/2)(Ftm - A.F1^-) + (1/2)(Fp - A.F1^+)
+          CmSite sm_, sp_; CmPrim Pm, Pp; double AFm[6], AFp[6], Fs[6];
+          cm_load_site<Nq, MOIST, GEOM>(p, e, nm, km, sm_); cm_eos<MOIST>(p, Ym, sm_, Pm);
+          cm_load_site<Nq, MOIST, GEOM>(p, nb, np_, kp, sp_); cm_eos<MOIST>(p, Yp, sp_, Pp);
+          cm_flux1_dir<MOIST>(Ym, Pm, A[0], A[1], A[2], AFm); cm_flux1_dir<MOIST>(Yp, Pp, A[0], A[1], A[2], AFp);
+          cm_hllc<MOIST>(Ym, Pm, AFm, Yp, Pp, AFp, A, sJ, Fs);
+#pragma unroll
+          for (int v = 0; v < NV; ++v) r[v] = Ftm[v] - (Fs[v] + 0.5 * (Ftm[v] - AFm[v]) + 0.5 * (Fp[v] - AFp[v]));
+        }
       } else {
         // free-slip wall (A6-A7): Rusanov against the mirrored state = [0; (p' + rho u_n (u_n + lambda)) n; 0; 0];
         // second-order normal fluxes vanish (R10) except the prescribed bottom energy flux
@@ -297,11 +315,26 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_ten
         cm_load_site<Nq, MOIST, GEOM>(p, e, nm, km, st);
         cm_eos<MOIST>(p, Ym, st, P);
         const double un = uAm / sJ;
-        const double lam = fabs(un) + cm_;
-        const double mom = P.pp + Ym[0] * un * (un + lam);
+        if (p.riemann == 0) {
+          const double lam = fabs(un) + cm_;
+          const double mom = P.pp + Ym[0] * un * (un + lam);
 #pragma unroll
-        for (int v = 0; v < NV; ++v) r[v] = Ftm[v];
-        r[1] -= mom * A[0]; r[2] -= mom * A[1]; r[3] -= mom * A[2];
+          for (int v = 0; v < NV; ++v) r[v] = Ftm[v];
+          r[1] -= mom * A[0]; r[2] -= mom * A[1]; r[3] -= mom * A[2];
+        } else {
+          // HLLC against the mirrored state (A6)-(A7); n.F2* = 0 at the wall (R10)
+          double Yg[6], AFm[6], AFg[6], Fs[6];
+          const double mn = 2.0 * (Ym[1] * A[0] + Ym[2] * A[1] + Ym[3] * A[2]) / (sJ * sJ);
+#pragma unroll
+          for (int v = 0; v < NV; ++v) Yg[v] = Ym[v];
+          Yg[1] -= mn * A[0]; Yg[2] -= mn * A[1]; Yg[3] -= mn * A[2];
+          CmPrim Pg = P;
+          Pg.u = Yg[1] * P.ir; Pg.v = Yg[2] * P.ir; Pg.w = Yg[3] * P.ir;
+          cm_flux1_dir<MOIST>(Ym, P, A[0], A[1], A[2], AFm); cm_flux1_dir<MOIST>(Yg, Pg, A[0], A[1], A[2], AFg);
+          cm_hllc<MOIST>(Ym, P, AFm, Yg, Pg, AFg, A, sJ, Fs);
+#pragma unroll
+          for (int v = 0; v < NV; ++v) r[v] = Ftm[v] - Fs[v];
+        }
         if (f == 4) r[4] += sJ * p.shf;
       }
       double* fb = fbuf + ((size_t)el * 6 * NF + ft) * NV;
@@ -361,6 +394,8 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_ten
     if (k == N) fs += fb[(5 * NF + i + Nq * j) * NV + v];
     double rhs = -invJ * (a - p.inv_w0 * fs);
     if (v == 3) rhs -= buoy;                                     // -(rho - rho_r) grad Phi   (eq. 4)
+    if (v >= 1 && v <= 3)                                        // Rayleigh sponge (A4); tau_s = 0 outside the layer
+      rhs -= taus * (Q_sh[((size_t)el * NV + v) * NP + n] - Q_sh[((size_t)el * NV) * NP + n] * p.urelax[v - 1]);
     if (!stage) {
       p.dQ[v * p.stride + idx] = rhs;
     } else {

@@ -130,11 +130,12 @@ __host__ __device__ constexpr int cm7_gidx(int d, int k) {
 
 // site (geopotential + reference column) from a z-table row held in shared memory
 __device__ __forceinline__ void cm7_site(const double* zrow, CmSite& s) {
-  s.Phi = zrow[0]; s.rho_r = zrow[1]; s.rhoe_r = zrow[2]; s.rhoq_r = zrow[3]; s.E_r = zrow[4]; s.q_r = zrow[5]; s.icvm_r = zrow[6];
+  s.Phi = zrow[0]; s.rho_r = zrow[1]; s.rhoe_r = zrow[2]; s.rhoq_r = zrow[3]; s.E_r = zrow[4]; s.q_r = zrow[5]; s.icvm_r = zrow[6]; s.taus = 0.0;
 }
 
 // primitives the gradient needs (u, v, w, h_tot, q): eq. (6)-(10), (13)-(14)
-template <bool MOIST>
+// RICH: also theta_v (eq. 40), stored behind the last regular gradient variable (index 5 moist, 4 dry)
+template <bool MOIST, bool RICH = false>
 __device__ __forceinline__ void cm7_eos_grad(const CmKP& p, const double* Y, double Phi, double* s) {
   const CmThermo& th = p.th;
   const double ir = cm_rcp(Y[0]);
@@ -147,6 +148,7 @@ __device__ __forceinline__ void cm7_eos_grad(const CmKP& p, const double* Y, dou
   const double E = Y[4] - K - Y[0] * Phi - rq * th.I_v0;
   const double pr = kappa * E + th.T_0 * (th.R_d * Y[0] + th.a * rq);
   s[0] = u; s[1] = v; s[2] = w; s[3] = (Y[4] + pr) * ir; s[4] = q;
+  if (RICH) s[MOIST ? 5 : 4] = cm_theta_v(th, pr, ir);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -423,7 +425,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
   if (node) {                                          // shared-memory copy of the z rows is only needed by the face tasks
     const double2* zr = reinterpret_cast<const double2*>(p.ztab + (size_t)(pos.ez * Nq + k_) * CM_ZTAB_W);
     const double2 a = __ldg(zr), b = __ldg(zr + 1), c = __ldg(zr + 2), d = __ldg(zr + 3);
-    st.Phi = a.x; st.rho_r = a.y; st.rhoe_r = b.x; st.rhoq_r = b.y; st.E_r = c.x; st.q_r = c.y; st.icvm_r = d.x;
+    st.Phi = a.x; st.rho_r = a.y; st.rhoe_r = b.x; st.rhoq_r = b.y; st.E_r = c.x; st.q_r = c.y; st.icvm_r = d.x; st.taus = d.y;
   }
   cm7_mbar_wait(mbar, 0);
 
@@ -490,6 +492,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
     for (int v = 0; v < NV; ++v) {
       double rhs = -p.invJ * (acc[v] - p.inv_w0 * lift[v]);
       if (v == 3) rhs -= buoy;                                   // -(rho - rho_r) grad Phi   (eq. 4)
+      if (v >= 1 && v <= 3) rhs -= st.taus * (Y[v] - Y[0] * p.urelax[v - 1]);   // Rayleigh sponge (A4); tau_s = 0 outside the layer
       if (MODE == 0) {
         __stcs(o1, rhs);
       } else {
@@ -650,16 +653,12 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
 #pragma unroll
         for (int c = 0; c < 3; ++c) __stcs(o + (size_t)(3 * v + c) * st, Gr[v][c]);
     } else {
-      // eq. (33)-(38): S, nu_t = (C_s Delta)^2 sqrt(2 S:S), D_t = nu_t / Pr_t; store tau, J + D, d_q
-      const double Sxx = Gr[0][0], Syy = Gr[1][1], Szz = Gr[2][2];
-      const double Sxy = 0.5 * (Gr[0][1] + Gr[1][0]), Sxz = 0.5 * (Gr[0][2] + Gr[2][0]), Syz = 0.5 * (Gr[1][2] + Gr[2][1]);
-      const double ss2 = Sxx * Sxx + Syy * Syy + Szz * Szz + 2.0 * (Sxy * Sxy + Sxz * Sxz + Syz * Syz);
-      const double nu = p.cs2delta2 * cm_sqrt(2.0 * ss2);
-      const double m2nu = -2.0 * nu, mDt = -nu * p.inv_Pr;
-      o[0] = m2nu * Sxx; o[st] = m2nu * Syy; o[2 * st] = m2nu * Szz;
-      o[3 * st] = m2nu * Sxy; o[4 * st] = m2nu * Sxz; o[5 * st] = m2nu * Syz;
-      o[6 * st] = mDt * Gr[3][0]; o[7 * st] = mDt * Gr[3][1]; o[8 * st] = mDt * Gr[3][2];
-      if (MOIST) { o[9 * st] = mDt * Gr[4][0]; o[10 * st] = mDt * Gr[4][1]; o[11 * st] = mDt * Gr[4][2]; }
+      // eq. (33)-(39): closure (cm_closure; the Richardson factor needs theta_v and is served by the other gradient
+      // kernels: cm_dg_setup routes richardson = 1 at these orders to the thread-per-node kernels)
+      double g[12];
+      cm_closure<MOIST>(p, Gr, p.cs2delta2, p.d2[0], p.d2[1], p.d2[2], 1.0, 0.0, g);
+#pragma unroll
+      for (int k = 0; k < C::NG; ++k) o[k * st] = g[k];
     }
   }
 }
@@ -674,7 +673,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg7<Nq, MOIST>:
 // ------------------------------------------------------------------------------------------------
 template <int Nq, bool MOIST> struct CmCfg9 {
   using C7 = CmCfg7<Nq, MOIST>;
-  static constexpr int GRAD_DOUBLES = (C7::NV + 3 * C7::NS) * C7::SLOT + 2;   // Q (then s in place), ds/dxi_d, mbarrier
+  static constexpr int GRAD_DOUBLES = (C7::NV + 3 * C7::NS + 1) * C7::SLOT + 2;   // Q (then s in place), ds/dxi_d, d theta_v/d zeta (eq. 40), mbarrier
   static constexpr size_t GRAD_SMEM = sizeof(double) * GRAD_DOUBLES;
   static constexpr bool OK = 3 * C7::NFP <= C7::THREADS;
   static constexpr int MINB_G = C7::cap(C7::fit(GRAD_SMEM), C7::cap(CM_G_REGTHREADS / C7::THREADS, 16));   // 896: >= 72 registers per thread
@@ -702,18 +701,19 @@ __device__ __forceinline__ bool cm9_line(int l, int& base, int& kline) {
   return true;
 }
 
-template <int Nq, bool MOIST, int D>
+template <int Nq, bool MOIST, int D, bool RICH>
 __device__ __forceinline__ void cm9_grad_line(const CmKP& p, const double* __restrict__ ss, double* __restrict__ dd,
                                               const double (&Yp)[2][6], const double (&Php)[2], int wallmask, int base) {
   using C = CmCfg7<Nq, MOIST>;
-  constexpr int N = Nq - 1, NS = C::NS, SLOT = C::SLOT, STR = Cm7Str<Nq, D>::value;
-  double dl[2][5];                                      // s* - s^- at the two ends (eq. 30-31: central flux)
+  // theta_v (eq. 40) needs its vertical derivative only: on flat bricks that is the zeta line
+  constexpr int N = Nq - 1, NS = C::NS + ((RICH && D == 2) ? 1 : 0), SLOT = C::SLOT, STR = Cm7Str<Nq, D>::value;
+  double dl[2][6];                                      // s* - s^- at the two ends (eq. 30-31: central flux)
 #pragma unroll
   for (int s = 0; s < 2; ++s) {
     const int nm = s ? base + N * STR : base;
     if (!((wallmask >> (2 * D + s)) & 1)) {
-      double sp[5];
-      cm7_eos_grad<MOIST>(p, Yp[s], Php[s], sp);
+      double sp[6];
+      cm7_eos_grad<MOIST, (RICH && D == 2)>(p, Yp[s], Php[s], sp);
 #pragma unroll
       for (int v = 0; v < NS; ++v) dl[s][v] = 0.5 * (sp[v] - ss[v * SLOT + nm]);
     } else {
@@ -741,14 +741,15 @@ __device__ __forceinline__ void cm9_grad_line(const CmKP& p, const double* __res
   }
 }
 
-template <int Nq, bool MOIST, bool RAW, bool GEM = false>
+// RICH: theta_v is a further gradient variable (its zeta derivative feeds the stability factor f_b of eq. 40)
+template <int Nq, bool MOIST, bool RAW, bool GEM = false, bool RICH = false>
 __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg9<Nq, MOIST>::MINB_G) cm9_gradient_kernel(const __grid_constant__ CmKP p) {
   using C = CmCfg7<Nq, MOIST>;
   constexpr int NF = C::NF, NP = C::NP, N = Nq - 1, NV = C::NV, NS = C::NS, SLOT = C::SLOT, NFP = C::NFP, THREADS = C::THREADS;
   extern __shared__ __align__(128) double smem7[];
   double* Qt = smem7;                                  // [NV][SLOT]      state, then the gradient variables in place
-  double* dt_ = Qt + NV * SLOT;                        // [3][NS][SLOT]   reference-space derivatives + lifted jumps
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(dt_ + 3 * NS * SLOT);
+  double* dt_ = Qt + NV * SLOT;                        // [3][NS][SLOT] (+1) reference-space derivatives + lifted jumps
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(dt_ + (3 * NS + 1) * SLOT);
 
   const int t = threadIdx.x;
   const Cm7Pos pos = cm7_position(p);
@@ -805,20 +806,20 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg9<Nq, MOIST>:
 
   // ---- phase 1: gradient variables of the own node, in place of the state
   if (node) {
-    double Y[6], s[5];
+    double Y[6], s[6];
 #pragma unroll
     for (int v = 0; v < NV; ++v) Y[v] = ss[v * SLOT + n];
-    cm7_eos_grad<MOIST>(p, Y, Phi, s);
+    cm7_eos_grad<MOIST, RICH>(p, Y, Phi, s);
 #pragma unroll
-    for (int v = 0; v < NS; ++v) ss[v * SLOT + n] = s[v];
+    for (int v = 0; v < NS + (RICH ? 1 : 0); ++v) ss[v * SLOT + n] = s[v];
   }
   __syncthreads();
 
   // ---- phase 2: one thread per line: contraction + lifted jumps at its two ends
   if (line) {
-    if (d == 0) cm9_grad_line<Nq, MOIST, 0>(p, ss, dd, Yp, Php, pos.wallmask, base);
-    else if (d == 1) cm9_grad_line<Nq, MOIST, 1>(p, ss, dd + NS * SLOT, Yp, Php, pos.wallmask, base);
-    else cm9_grad_line<Nq, MOIST, 2>(p, ss, dd + 2 * NS * SLOT, Yp, Php, pos.wallmask, base);
+    if (d == 0) cm9_grad_line<Nq, MOIST, 0, RICH>(p, ss, dd, Yp, Php, pos.wallmask, base);
+    else if (d == 1) cm9_grad_line<Nq, MOIST, 1, RICH>(p, ss, dd + NS * SLOT, Yp, Php, pos.wallmask, base);
+    else cm9_grad_line<Nq, MOIST, 2, RICH>(p, ss, dd + 2 * NS * SLOT, Yp, Php, pos.wallmask, base);
   }
   __syncthreads();
 
@@ -839,16 +840,13 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg9<Nq, MOIST>:
 #pragma unroll
         for (int c = 0; c < 3; ++c) __stcs(o + (size_t)(3 * v + c) * st, Gr[v][c]);
     } else {
-      // eq. (33)-(38): S, nu_t = (C_s Delta)^2 sqrt(2 S:S), D_t = nu_t / Pr_t; store tau, J + D, d_q
-      const double Sxx = Gr[0][0], Syy = Gr[1][1], Szz = Gr[2][2];
-      const double Sxy = 0.5 * (Gr[0][1] + Gr[1][0]), Sxz = 0.5 * (Gr[0][2] + Gr[2][0]), Syz = 0.5 * (Gr[1][2] + Gr[2][1]);
-      const double ss2 = Sxx * Sxx + Syy * Syy + Szz * Szz + 2.0 * (Sxy * Sxy + Sxz * Sxz + Syz * Syz);
-      const double nu = p.cs2delta2 * cm_sqrt(2.0 * ss2);
-      const double m2nu = -2.0 * nu, mDt = -nu * p.inv_Pr;
-      o[0] = m2nu * Sxx; o[st] = m2nu * Syy; o[2 * st] = m2nu * Szz;
-      o[3 * st] = m2nu * Sxy; o[4 * st] = m2nu * Sxz; o[5 * st] = m2nu * Syz;
-      o[6 * st] = mDt * Gr[3][0]; o[7 * st] = mDt * Gr[3][1]; o[8 * st] = mDt * Gr[3][2];
-      if (MOIST) { o[9 * st] = mDt * Gr[4][0]; o[10 * st] = mDt * Gr[4][1]; o[11 * st] = mDt * Gr[4][2]; }
+      // eq. (33)-(40): closure (cm_closure); store tau, J + D, d_q
+      double thv = 1.0, dthv = 0.0;
+      if (RICH) { thv = ss[NS * SLOT + n]; dthv = (p.cA[2] * p.invJ) * dd[(3 * NS) * SLOT + n]; }
+      double g[12];
+      cm_closure<MOIST>(p, Gr, p.cs2delta2, p.d2[0], p.d2[1], p.d2[2], thv, dthv, g);
+#pragma unroll
+      for (int k = 0; k < C::NG; ++k) o[k * st] = g[k];
     }
   }
 }

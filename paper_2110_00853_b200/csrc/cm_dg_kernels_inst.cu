@@ -1,5 +1,6 @@
 // cm_dg_kernels_inst.cu -- instantiates the hot kernels for ONE polynomial order (compile with -DCM_NQ=<N+1>),
 // so that the orders build in parallel.  Exposes cm_launch_gradient_nq<NQ> / cm_launch_tendency_nq<NQ>.
+#include <atomic>
 #include "cm_dg_kernels2.cuh"
 #include "cm_dg_kernels7.cuh"
 #include "cm_dg_kernels10.cuh"
@@ -13,10 +14,10 @@
 
 namespace {
 
-template <int Nq, bool MOIST>
+template <int Nq, bool MOIST, bool RICH>
 constexpr size_t grad2_smem() {
   using C = CmCfg2<Nq>;
-  constexpr int NS = MOIST ? 5 : 4;
+  constexpr int NS = (MOIST ? 5 : 4) + (RICH ? 1 : 0);
   return sizeof(double) * (size_t)(4 * C::EPB * NS * C::NP + C::EPB * 6 * C::NF * NS);
 }
 template <int Nq, bool MOIST>
@@ -26,39 +27,12 @@ constexpr size_t tend2_smem() {
   return sizeof(double) * (size_t)(4 * C::EPB * NV * C::NP + C::EPB * C::NP + C::EPB * 6 * C::NF * NV);
 }
 
-template <typename K>
-cudaError_t configure(K kernel, size_t smem, bool& configured) {
-  if (configured) return cudaSuccess;
-  cudaError_t err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (err == cudaSuccess) err = cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-  if (err == cudaSuccess) configured = true;
-  return err;
-}
+// Per-kernel launch state, kept PER DEVICE: cudaFuncSetAttribute and the occupancy query act on the current device only.
+// Concurrent first launches from several host threads at worst repeat the (idempotent) configuration.
+constexpr int CM_MAX_DEVICES = 64;
+struct LaunchState { std::atomic<bool> configured[CM_MAX_DEVICES]; std::atomic<int> wave[CM_MAX_DEVICES]; };
 
-template <int Nq, bool MOIST, int GEOM>
-cudaError_t launch_grad2(const CmKP& kp, cudaStream_t st) {
-  using C = CmCfg2<Nq>;
-  static bool configured = false;
-  constexpr size_t smem = grad2_smem<Nq, MOIST>();
-  cudaError_t err = configure(cm2_gradient_kernel<Nq, MOIST, GEOM>, smem, configured);
-  if (err != cudaSuccess) return err;
-  const int blocks = (kp.Ne + C::EPB - 1) / C::EPB;
-  cm2_gradient_kernel<Nq, MOIST, GEOM><<<blocks, C::THREADS, smem, st>>>(kp);
-  return cudaGetLastError();
-}
-
-template <int Nq, bool MOIST, int GEOM>
-cudaError_t launch_tend2(const CmKP& kp, cudaStream_t st) {
-  using C = CmCfg2<Nq>;
-  static bool configured = false;
-  constexpr size_t smem = tend2_smem<Nq, MOIST>();
-  cudaError_t err = configure(cm2_tendency_kernel<Nq, MOIST, GEOM>, smem, configured);
-  if (err != cudaSuccess) return err;
-  const int blocks = (kp.Ne + C::EPB - 1) / C::EPB;
-  cm2_tendency_kernel<Nq, MOIST, GEOM><<<blocks, C::THREADS, smem, st>>>(kp);
-  return cudaGetLastError();
-}
-
+inline int current_device() { int dev = 0; cudaGetDevice(&dev); return (dev >= 0 && dev < CM_MAX_DEVICES) ? dev : 0; }
 
 // one wave of resident CTAs = the L2 prefetch distance of the flat kernels (CmKP::ahead < 0)
 template <typename K>
@@ -69,29 +43,69 @@ int wave_size(K kernel, int threads, size_t smem) {
   return sms * per_sm;
 }
 
-template <int Nq, bool MOIST, bool RAW, bool GEM = false>
+// sets the shared-memory attributes of `kernel` on the current device once; returns the device's wave size in *wave
+template <typename K>
+cudaError_t configure(K kernel, size_t smem, LaunchState& ls, int threads = 0, int* wave = nullptr) {
+  const int dev = current_device();
+  if (!ls.configured[dev].load(std::memory_order_acquire)) {
+    cudaError_t err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err == cudaSuccess) err = cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (err != cudaSuccess) return err;
+    if (threads > 0) ls.wave[dev].store(wave_size(kernel, threads, smem), std::memory_order_relaxed);
+    ls.configured[dev].store(true, std::memory_order_release);
+  }
+  if (wave) *wave = ls.wave[dev].load(std::memory_order_relaxed);
+  return cudaSuccess;
+}
+
+template <int Nq, bool MOIST, int GEOM, bool RICH>
+cudaError_t launch_grad2r(const CmKP& kp, cudaStream_t st) {
+  using C = CmCfg2<Nq>;
+  static LaunchState ls;
+  constexpr size_t smem = grad2_smem<Nq, MOIST, RICH>();
+  cudaError_t err = configure(cm2_gradient_kernel<Nq, MOIST, GEOM, RICH>, smem, ls);
+  if (err != cudaSuccess) return err;
+  const int blocks = (kp.Ne + C::EPB - 1) / C::EPB;
+  cm2_gradient_kernel<Nq, MOIST, GEOM, RICH><<<blocks, C::THREADS, smem, st>>>(kp);
+  return cudaGetLastError();
+}
+template <int Nq, bool MOIST, int GEOM>
+cudaError_t launch_grad2(const CmKP& kp, cudaStream_t st) {
+  // the Richardson factor (eq. 40) needs theta_v as a further gradient variable; the raw-gradient mode does not
+  if (kp.richardson && kp.mode == 0) return launch_grad2r<Nq, MOIST, GEOM, true>(kp, st);
+  return launch_grad2r<Nq, MOIST, GEOM, false>(kp, st);
+}
+
+template <int Nq, bool MOIST, int GEOM>
+cudaError_t launch_tend2(const CmKP& kp, cudaStream_t st) {
+  using C = CmCfg2<Nq>;
+  static LaunchState ls;
+  constexpr size_t smem = tend2_smem<Nq, MOIST>();
+  cudaError_t err = configure(cm2_tendency_kernel<Nq, MOIST, GEOM>, smem, ls);
+  if (err != cudaSuccess) return err;
+  const int blocks = (kp.Ne + C::EPB - 1) / C::EPB;
+  cm2_tendency_kernel<Nq, MOIST, GEOM><<<blocks, C::THREADS, smem, st>>>(kp);
+  return cudaGetLastError();
+}
+
+
+template <int Nq, bool MOIST, bool RAW, bool GEM = false, bool RICH = false>
 cudaError_t launch_grad7(const CmKP& kp, cudaStream_t st) {
   using C = CmCfg7<Nq, MOIST>;
-  static bool configured = false;
+  static LaunchState ls;
   const dim3 grid(kp.gPY * kp.gL, kp.gEz, kp.gNXC * kp.gNYP);
+  int wave = 0;
+  CmKP k2 = kp;
   if constexpr (CmCfg9<Nq, MOIST>::OK) {
     // every line task has its own thread: register-staged traces (cm9_gradient_kernel)
     constexpr size_t smem = CmCfg9<Nq, MOIST>::GRAD_SMEM;
-    static int wave = 0;
-    const bool first = !configured;
-    cudaError_t err = configure(cm9_gradient_kernel<Nq, MOIST, RAW, GEM>, smem, configured);
+    cudaError_t err = configure(cm9_gradient_kernel<Nq, MOIST, RAW, GEM, RICH>, smem, ls, C::THREADS, &wave);
     if (err != cudaSuccess) return err;
-    if (first) wave = wave_size(cm9_gradient_kernel<Nq, MOIST, RAW, GEM>, C::THREADS, smem);
-    CmKP k2 = kp;
     if (k2.ahead < 0) k2.ahead = wave;
-    cm9_gradient_kernel<Nq, MOIST, RAW, GEM><<<grid, C::THREADS, smem, st>>>(k2);
+    cm9_gradient_kernel<Nq, MOIST, RAW, GEM, RICH><<<grid, C::THREADS, smem, st>>>(k2);
   } else {
-    static int wave = 0;
-    const bool first = !configured;
-    cudaError_t err = configure(cm7_gradient_kernel<Nq, MOIST, RAW, GEM>, C::GRAD_SMEM, configured);
+    cudaError_t err = configure(cm7_gradient_kernel<Nq, MOIST, RAW, GEM>, C::GRAD_SMEM, ls, C::THREADS, &wave);
     if (err != cudaSuccess) return err;
-    if (first) wave = wave_size(cm7_gradient_kernel<Nq, MOIST, RAW, GEM>, C::THREADS, C::GRAD_SMEM);
-    CmKP k2 = kp;
     if (k2.ahead < 0) k2.ahead = wave;
     cm7_gradient_kernel<Nq, MOIST, RAW, GEM><<<grid, C::THREADS, C::GRAD_SMEM, st>>>(k2);
   }
@@ -101,12 +115,10 @@ cudaError_t launch_grad7(const CmKP& kp, cudaStream_t st) {
 template <int Nq, bool MOIST, bool SGS, int MODE>
 cudaError_t launch_tend7(const CmKP& kp, cudaStream_t st) {
   using C = CmCfg7<Nq, MOIST>;
-  static bool configured = false;
-  static int wave = 0;
-  const bool first = !configured;
-  cudaError_t err = configure(cm7_tendency_kernel<Nq, MOIST, SGS, MODE>, C::TEND_SMEM, configured);
+  static LaunchState ls;
+  int wave = 0;
+  cudaError_t err = configure(cm7_tendency_kernel<Nq, MOIST, SGS, MODE>, C::TEND_SMEM, ls, C::THREADS, &wave);
   if (err != cudaSuccess) return err;
-  if (first) wave = wave_size(cm7_tendency_kernel<Nq, MOIST, SGS, MODE>, C::THREADS, C::TEND_SMEM);
   CmKP k2 = kp;
   if (k2.ahead < 0) k2.ahead = wave;
   cm7_tendency_kernel<Nq, MOIST, SGS, MODE><<<dim3(kp.gPY * kp.gL, kp.gEz, kp.gNXC * kp.gNYP), C::THREADS, C::TEND_SMEM, st>>>(k2);
@@ -125,8 +137,8 @@ cudaError_t launch_tend10(const CmKP& kp, cudaStream_t st) {
   using C = CmCfg7<Nq, MOIST>;
   using R = CmCfg10<Nq, MOIST, MODE>;
   if constexpr (CmCfg10<Nq, true, 1>::OK) {   // one predicate per order: G / residual layouts must agree across all launches of a ctx
-    static bool configured = false;
-    cudaError_t err = configure(cm10_tendency_kernel<Nq, MOIST, SGS, MODE>, R::SMEM, configured);
+    static LaunchState ls;
+    cudaError_t err = configure(cm10_tendency_kernel<Nq, MOIST, SGS, MODE>, R::SMEM, ls);
     if (err != cudaSuccess) return err;
     const dim3 grid(kp.gPY * (kp.gL / kp.gS), kp.gEz, kp.gNXC * kp.gNYP);
     cm10_tendency_kernel<Nq, MOIST, SGS, MODE><<<grid, C::THREADS + 32, R::SMEM, st>>>(kp);
@@ -147,8 +159,12 @@ cudaError_t launch_tend10m(const CmKP& kp, cudaStream_t st) {
 cudaError_t CM_CAT(cm_launch_gradient_nq, CM_NQ)(const CmKP& kp, int moist, int general, int variant, cudaStream_t st) {
   if ((variant == 7 || variant == 10) && !general) {
     if (kp.mode == 1) return moist ? launch_grad7<CM_NQ, true, true>(kp, st) : launch_grad7<CM_NQ, false, true>(kp, st);
-    if (variant == 10 && CmCfg10<CM_NQ, true, 1>::OK)    // the row-sweep tendency kernel reads G element-major
+    // (cm_dg_setup routes richardson = 1 to the thread-per-node kernels at the orders without a cm9 kernel)
+    if (variant == 10 && CmCfg10<CM_NQ, true, 1>::OK) {   // the row-sweep tendency kernel reads G element-major
+      if (kp.richardson) return moist ? launch_grad7<CM_NQ, true, false, true, true>(kp, st) : launch_grad7<CM_NQ, false, false, true, true>(kp, st);
       return moist ? launch_grad7<CM_NQ, true, false, true>(kp, st) : launch_grad7<CM_NQ, false, false, true>(kp, st);
+    }
+    if (kp.richardson) return moist ? launch_grad7<CM_NQ, true, false, false, true>(kp, st) : launch_grad7<CM_NQ, false, false, false, true>(kp, st);
     return moist ? launch_grad7<CM_NQ, true, false>(kp, st) : launch_grad7<CM_NQ, false, false>(kp, st);
   }
   if (moist) return general ? launch_grad2<CM_NQ, true, 1>(kp, st) : launch_grad2<CM_NQ, true, 0>(kp, st);

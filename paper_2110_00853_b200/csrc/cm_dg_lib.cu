@@ -81,6 +81,37 @@ void lgl_operators(int N, double* xi, double* w, double (*D)[CM_MAXNQ]) {
   }
 }
 
+// 1-D nodal matrix of the exponential filter of eq. (52): F = V diag(sigma) V^-1 with V_ij = P_j(xi_i) (Legendre modes at
+// the LGL nodes) and sigma_j = exp(-alpha (j / N)^s) (eta = mode number / polynomial order, reading R26); long double.
+void filter_operator(int N, const double* xi, int order, double alpha, double (*F)[CM_MAXNQ]) {
+  const int Nq = N + 1;
+  long double A[CM_MAXNQ][2 * CM_MAXNQ], V[CM_MAXNQ][CM_MAXNQ];
+  for (int i = 0; i < Nq; ++i) {
+    long double a = 1.0L, b = xi[i];
+    for (int j = 0; j < Nq; ++j) {
+      V[i][j] = (j == 0) ? a : b;
+      if (j >= 1) { long double cnx = ((2 * j + 1) * (long double)xi[i] * b - j * a) / (j + 1); a = b; b = cnx; }
+    }
+  }
+  for (int i = 0; i < Nq; ++i)
+    for (int j = 0; j < Nq; ++j) { A[i][j] = V[i][j]; A[i][Nq + j] = (i == j) ? 1.0L : 0.0L; }
+  for (int col = 0; col < Nq; ++col) {
+    int piv = col;
+    for (int r = col + 1; r < Nq; ++r) if (fabsl(A[r][col]) > fabsl(A[piv][col])) piv = r;
+    for (int j = 0; j < 2 * Nq; ++j) std::swap(A[col][j], A[piv][j]);
+    const long double d = A[col][col];
+    for (int j = 0; j < 2 * Nq; ++j) A[col][j] /= d;
+    for (int r = 0; r < Nq; ++r)
+      if (r != col) { const long double f = A[r][col]; for (int j = 0; j < 2 * Nq; ++j) A[r][j] -= f * A[col][j]; }
+  }
+  for (int i = 0; i < Nq; ++i)
+    for (int j = 0; j < Nq; ++j) {
+      long double acc = 0.0L;
+      for (int m = 0; m < Nq; ++m) acc += V[i][m] * expl(-(long double)alpha * powl((long double)m / N, order)) * A[m][Nq + j];
+      F[i][j] = (double)acc;
+    }
+}
+
 // ------------------------------------------------------------------ small kernels
 struct GeoArgs {
   int Nq, Np, geom;
@@ -92,6 +123,8 @@ struct GeoArgs {
   const double* xyz_user; // geom 2: [3][stride] library order
   double xi[CM_MAXNQ], w[CM_MAXNQ], D[CM_MAXNQ][CM_MAXNQ];
   double cs, grav;
+  int N, metric_form;          // polynomial order; 0 cross-product | 1 curl-invariant metric terms
+  double sp_alpha, sp_zs; int sp_gamma;   // Rayleigh sponge (A5)
 };
 
 __device__ inline void node_xyz(const GeoArgs& a, long long e, int n, double* X) {
@@ -119,11 +152,19 @@ __global__ void coords_kernel(const __grid_constant__ GeoArgs a, double* __restr
 
 // metric terms of one element per block: geo = Ja[9], 1/J, z, (C_s Delta)^2; chk[e] = {min J, metric-identity
 // residual / max|Ja|, min node spacing}
+__device__ inline double sponge_tau(double alpha, double zs, int gamma, double ztop, double z) {
+  // tau_s = alpha sin^gamma(pi/2 (z - z_s) / (z_top - z_s)) for z > z_s   (A5 with reading R18)
+  if (!(alpha > 0.0) || !(z > zs)) return 0.0;
+  return alpha * pow(sin(0.5 * 3.14159265358979323846 * (z - zs) / (ztop - zs)), (double)gamma);
+}
+
 __global__ void metrics_kernel(const __grid_constant__ GeoArgs a, double* __restrict__ geo, double* __restrict__ chk) {
   extern __shared__ double sh[];
   double* X = sh;                 // [3][Np]
   double* JA = sh + 3 * a.Np;     // [9][Np]
-  double* red = JA + 9 * a.Np;    // [3][blockDim]
+  double* DX = JA + 9 * a.Np;     // [9][Np]  d x_c / d xi_d at [3 d + c]  (curl form)
+  double* V = DX + 9 * a.Np;      // [3][Np]  X_l d X_m / d xi_d           (curl form)
+  double* red = V + 3 * a.Np;     // [4][blockDim]
   const long long e = blockIdx.x;
   const int Nq = a.Nq, Np = a.Np;
   for (int n = threadIdx.x; n < Np; n += blockDim.x) {
@@ -142,17 +183,21 @@ __global__ void metrics_kernel(const __grid_constant__ GeoArgs a, double* __rest
         xs[d] += a.D[j][m] * (X[d * Np + i + Nq * (m + Nq * k)] - X[d * Np]);
         xt[d] += a.D[k][m] * (X[d * Np + i + Nq * (j + Nq * m)] - X[d * Np]);
       }
+    for (int d = 0; d < 3; ++d) { DX[d * Np + n] = xr[d]; DX[(3 + d) * Np + n] = xs[d]; DX[(6 + d) * Np + n] = xt[d]; }
     double A[9];
     A[0] = xs[1] * xt[2] - xs[2] * xt[1]; A[1] = xs[2] * xt[0] - xs[0] * xt[2]; A[2] = xs[0] * xt[1] - xs[1] * xt[0];
     A[3] = xt[1] * xr[2] - xt[2] * xr[1]; A[4] = xt[2] * xr[0] - xt[0] * xr[2]; A[5] = xt[0] * xr[1] - xt[1] * xr[0];
     A[6] = xr[1] * xs[2] - xr[2] * xs[1]; A[7] = xr[2] * xs[0] - xr[0] * xs[2]; A[8] = xr[0] * xs[1] - xr[1] * xs[0];
     const double J = xr[0] * A[0] + xr[1] * A[1] + xr[2] * A[2];
     const long long idx = e * Np + n;
-    for (int m = 0; m < 9; ++m) { geo[m * a.stride + idx] = A[m]; JA[m * Np + n] = A[m]; amax = fmax(amax, fabs(A[m])); }
+    for (int m = 0; m < 9; ++m) JA[m * Np + n] = A[m];
     geo[9 * a.stride + idx] = 1.0 / J;
     geo[10 * a.stride + idx] = X[2 * Np + n];
     const double delta = cbrt(8.0 * J) / (Nq - 1);              // filter width, reading R7
     geo[11 * a.stride + idx] = (a.cs * delta) * (a.cs * delta);
+    const double dm[3] = {2.0 * fabs(xr[0]) / a.N, 2.0 * fabs(xs[1]) / a.N, 2.0 * fabs(xt[2]) / a.N};   // mixing lengths (eq. 39c, R24)
+    for (int m = 0; m < 3; ++m) geo[(12 + m) * a.stride + idx] = dm[m] * dm[m];
+    geo[15 * a.stride + idx] = sponge_tau(a.sp_alpha, a.sp_zs, a.sp_gamma, a.hi[2], X[2 * Np + n]);
     minJ = fmin(minJ, J);
     const int nb[3] = {(i + 1 < Nq) ? n + 1 : -1, (j + 1 < Nq) ? n + Nq : -1, (k + 1 < Nq) ? n + Nq * Nq : -1};
     for (int d = 0; d < 3; ++d)
@@ -162,6 +207,33 @@ __global__ void metrics_kernel(const __grid_constant__ GeoArgs a, double* __rest
         mindx = fmin(mindx, sqrt(s));
       }
   }
+  __syncthreads();
+  if (a.metric_form == 1) {
+    // curl-invariant form (Kopriva 2006): Ja^i_n = -xhat_i . curl_xi( I_N( X_l grad_xi X_m ) ), (n, m, l) cyclic: the
+    // discrete metric identities then hold on fully 3-D warps
+    for (int nn = 0; nn < 3; ++nn) {
+      const int mm = (nn + 1) % 3, ll = (nn + 2) % 3;
+      for (int n = threadIdx.x; n < Np; n += blockDim.x)
+        for (int d = 0; d < 3; ++d) V[d * Np + n] = (X[ll * Np + n] - X[ll * Np]) * DX[(3 * d + mm) * Np + n];
+      __syncthreads();
+      for (int n = threadIdx.x; n < Np; n += blockDim.x) {
+        const int i = n % Nq, j = (n / Nq) % Nq, k = n / (Nq * Nq);
+        double dV[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};      // dV[a][d] = d V_d / d xi_a
+        for (int m = 0; m < Nq; ++m)
+          for (int d = 0; d < 3; ++d) {
+            dV[0][d] += a.D[i][m] * V[d * Np + m + Nq * (j + Nq * k)];
+            dV[1][d] += a.D[j][m] * V[d * Np + i + Nq * (m + Nq * k)];
+            dV[2][d] += a.D[k][m] * V[d * Np + i + Nq * (j + Nq * m)];
+          }
+        JA[(0 + nn) * Np + n] = -(dV[1][2] - dV[2][1]);
+        JA[(3 + nn) * Np + n] = -(dV[2][0] - dV[0][2]);
+        JA[(6 + nn) * Np + n] = -(dV[0][1] - dV[1][0]);
+      }
+      __syncthreads();
+    }
+  }
+  for (int n = threadIdx.x; n < Np; n += blockDim.x)
+    for (int m = 0; m < 9; ++m) { const double v = JA[m * Np + n]; geo[m * a.stride + e * Np + n] = v; amax = fmax(amax, fabs(v)); }
   __syncthreads();
   double res = 0.0;
   for (int n = threadIdx.x; n < Np; n += blockDim.x) {
@@ -174,6 +246,7 @@ __global__ void metrics_kernel(const __grid_constant__ GeoArgs a, double* __rest
       res = fmax(res, fabs(r));
     }
   }
+  __syncthreads();
   red[threadIdx.x] = minJ; red[blockDim.x + threadIdx.x] = res; red[2 * blockDim.x + threadIdx.x] = mindx;
   double* red4 = red + 3 * blockDim.x; red4[threadIdx.x] = amax;
   __syncthreads();
@@ -244,6 +317,57 @@ __global__ void diag_kernel(const __grid_constant__ DiagArgs a, double* __restri
   }
 }
 
+// eq. (52): Q <- Q_ref + (F x F x F)(Q - Q_ref), one element per block, one field at a time through shared memory
+struct FilterArgs {
+  int Nq, Np, nvar, general, use_ref;
+  long long stride;
+  double* Q; const int* erow; const double* ztab; const double* ref;
+  double F[CM_MAXNQ][CM_MAXNQ];
+};
+
+__global__ void filter_kernel(const __grid_constant__ FilterArgs a) {
+  extern __shared__ double sh[];
+  double* u = sh; double* w = sh + a.Np;
+  const long long e = blockIdx.x;
+  const int Nq = a.Nq, Np = a.Np;
+  for (int v = 0; v < a.nvar; ++v) {
+    for (int n = threadIdx.x; n < Np; n += blockDim.x) {
+      const long long idx = e * Np + n;
+      double r = 0.0;
+      if (a.use_ref && (v == 0 || v >= 4)) {
+        const int col = (v == 0) ? 0 : (v == 4) ? 1 : 2;                   // rho_r, rhoe_r, rhoq_r
+        r = a.general ? a.ref[col * a.stride + idx] : a.ztab[(long long)(a.erow[e] + n / (Nq * Nq)) * CM_ZTAB_W + 1 + col];
+      }
+      u[n] = a.Q[v * a.stride + idx] - r;
+    }
+    __syncthreads();
+    for (int n = threadIdx.x; n < Np; n += blockDim.x) {
+      const int i = n % Nq, jk = n / Nq;
+      double t = 0.0; for (int m = 0; m < Nq; ++m) t += a.F[i][m] * u[m + Nq * jk];
+      w[n] = t;
+    }
+    __syncthreads();
+    for (int n = threadIdx.x; n < Np; n += blockDim.x) {
+      const int i = n % Nq, j = (n / Nq) % Nq, k = n / (Nq * Nq);
+      double t = 0.0; for (int m = 0; m < Nq; ++m) t += a.F[j][m] * w[i + Nq * (m + Nq * k)];
+      u[n] = t;
+    }
+    __syncthreads();
+    for (int n = threadIdx.x; n < Np; n += blockDim.x) {
+      const int ij = n % (Nq * Nq), k = n / (Nq * Nq);
+      double t = 0.0; for (int m = 0; m < Nq; ++m) t += a.F[k][m] * u[ij + Nq * Nq * m];
+      const long long idx = e * Np + n;
+      double r = 0.0;
+      if (a.use_ref && (v == 0 || v >= 4)) {
+        const int col = (v == 0) ? 0 : (v == 4) ? 1 : 2;
+        r = a.general ? a.ref[col * a.stride + idx] : a.ztab[(long long)(a.erow[e] + k) * CM_ZTAB_W + 1 + col];
+      }
+      a.Q[v * a.stride + idx] = r + t;
+    }
+    __syncthreads();
+  }
+}
+
 }  // namespace
 
 struct cm_dg_ctx {
@@ -253,8 +377,9 @@ struct cm_dg_ctx {
                      // 2: thread-per-node kernels (cm_dg_kernels2.cuh; any geometry); cm_dg_tuning::kernel selects
   int64_t Ne, stride;
   cudaStream_t st;
+  int device = 0;      // the CUDA device the ctx was set up on: every entry point rejects calls made from another one
   std::vector<int32_t> lex_of_elem;
-  double xi[CM_MAXNQ], w[CM_MAXNQ], D[CM_MAXNQ][CM_MAXNQ];
+  double xi[CM_MAXNQ], w[CM_MAXNQ], D[CM_MAXNQ][CM_MAXNQ], Filt[CM_MAXNQ][CM_MAXNQ];
   double h[3], min_node_dx;
   size_t em_bytes_per_field = 0;   // bytes per field of G and of the residual (field-major or element-major layout)
   // device
@@ -282,6 +407,16 @@ void free_ctx(cm_dg_ctx* c) {
   delete c;
 }
 
+// Every computing entry point starts here: the ctx is bound to the device that was current in cm_dg_setup.
+int enter(const cm_dg_ctx* c, const char* who) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return fail(CM_DG_ECUDA, std::string(who) + ": cudaGetDevice failed");
+  if (dev != c->device)
+    return fail(CM_DG_ESTATE, std::string(who) + ": the ctx belongs to CUDA device " + std::to_string(c->device) +
+                              " but the current device is " + std::to_string(dev));
+  return CM_DG_OK;
+}
+
 GeoArgs geo_args(const cm_dg_ctx* c) {
   GeoArgs a;
   a.Nq = c->Nq; a.Np = c->Np; a.geom = c->prm.geom; a.Ne = c->Ne; a.stride = c->stride;
@@ -289,6 +424,8 @@ GeoArgs geo_args(const cm_dg_ctx* c) {
   a.lex = c->d_lex; a.zsfc = c->d_zsfc; a.xyz_user = c->d_xyz_user;
   for (int i = 0; i < CM_MAXNQ; ++i) { a.xi[i] = c->xi[i]; a.w[i] = c->w[i]; for (int j = 0; j < CM_MAXNQ; ++j) a.D[i][j] = c->D[i][j]; }
   a.cs = c->prm.C_s; a.grav = c->prm.grav;
+  a.N = c->N; a.metric_form = c->prm.metric_form;
+  a.sp_alpha = c->prm.sponge_alpha; a.sp_zs = c->prm.sponge_zs; a.sp_gamma = c->prm.sponge_gamma;
   return a;
 }
 
@@ -367,7 +504,16 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   if (p->geom == 2 && !p->xyz) return fail(CM_DG_EINVAL, "cm_dg_setup: geom == 2 needs xyz");
   if (p->use_ref && (!p->ref_rho || !p->ref_rhoe || (p->nvar == 6 && !p->ref_rhoq)))
     return fail(CM_DG_EINVAL, "cm_dg_setup: use_ref needs ref_rho, ref_rhoe (and ref_rhoq when nvar == 6)");
+  if (p->sgs < 0 || p->sgs > 2) return fail(CM_DG_EINVAL, "cm_dg_setup: sgs must be 0 (inviscid), 1 (Smagorinsky-Lilly) or 2 (Vreman)");
   if (p->sgs && !(p->Pr_t > 0.0)) return fail(CM_DG_EINVAL, "cm_dg_setup: Pr_t must be positive");
+  if (p->richardson != 0 && p->richardson != 1) return fail(CM_DG_EINVAL, "cm_dg_setup: richardson must be 0 or 1");
+  if (p->richardson && !p->sgs) return fail(CM_DG_EINVAL, "cm_dg_setup: richardson = 1 needs an eddy-viscosity closure (sgs != 0)");
+  if (p->p_0 < 0.0) return fail(CM_DG_EINVAL, "cm_dg_setup: p_0 must be positive (0 = 1e5 Pa)");
+  if (p->riemann != 0 && p->riemann != 1) return fail(CM_DG_EINVAL, "cm_dg_setup: riemann must be 0 (Rusanov) or 1 (HLLC)");
+  if (p->metric_form != 0 && p->metric_form != 1) return fail(CM_DG_EINVAL, "cm_dg_setup: metric_form must be 0 or 1");
+  if (p->filter_order < 0 || p->filter_alpha < 0.0) return fail(CM_DG_EINVAL, "cm_dg_setup: filter_order and filter_alpha must be >= 0");
+  if (p->sponge_alpha < 0.0 || p->sponge_gamma < 0) return fail(CM_DG_EINVAL, "cm_dg_setup: sponge_alpha and sponge_gamma must be >= 0");
+  if (p->sponge_alpha > 0.0 && !(p->sponge_zs < p->hi[2])) return fail(CM_DG_EINVAL, "cm_dg_setup: the sponge must start below hi[2]");
   if (!(p->c_vd > 0.0) || !(p->R_d > 0.0)) return fail(CM_DG_EINVAL, "cm_dg_setup: R_d and c_vd must be positive");
   const int64_t Ne = (int64_t)p->ne[0] * p->ne[1] * p->ne[2];
   const int Nq = p->N + 1, Np = Nq * Nq * Nq;
@@ -380,14 +526,20 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   cm_dg_ctx* c = new cm_dg_ctx();
   c->prm = *p;
   c->prm.zsfc_nodes = nullptr; c->prm.xyz = nullptr; c->prm.ref_rho = c->prm.ref_rhoe = c->prm.ref_rhoq = nullptr;
+  if (c->prm.p_0 == 0.0) c->prm.p_0 = 1.0e5;
+  if (c->prm.sponge_gamma == 0) c->prm.sponge_gamma = 2;
+  if (c->prm.filter_alpha == 0.0) c->prm.filter_alpha = 36.0436533891172;   // -log(2^-52)
   c->N = p->N; c->Nq = Nq; c->Np = Np; c->nvar = p->nvar; c->moist = (p->nvar == 6);
   c->ngrad = c->moist ? 12 : 9;
   c->Ne = Ne;
   c->stride = ((Ne * Np + 1 + 31) / 32) * 32;   // >= Ne*Np + 1: the bulk-TMA tile fetch of the last element reads one double past it
   c->st = (cudaStream_t)cuda_stream;
+  if (cudaGetDevice(&c->device) != cudaSuccess) { delete c; return fail(CM_DG_ECUDA, "cm_dg_setup: cudaGetDevice failed"); }
   for (int d = 0; d < 3; ++d) c->h[d] = (p->hi[d] - p->lo[d]) / p->ne[d];
   std::memset(c->D, 0, sizeof(c->D));
   lgl_operators(c->N, c->xi, c->w, c->D);
+  std::memset(c->Filt, 0, sizeof(c->Filt));
+  if (c->prm.filter_order > 0) filter_operator(c->N, c->xi, c->prm.filter_order, c->prm.filter_alpha, c->Filt);
 
   // ---- element order (library order = launch order of the CTA-per-element kernels)
   // e = ((((ey / PY) * NXC + ex / L) * Ez + ez) * PY + ey % PY) * L + ex % L with L | Ex, PY | Ey: consecutive CTAs
@@ -446,10 +598,13 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
           }
       }
   }
-  c->general = (p->geom != 0 || (p->use_ref && !ref_z_only)) ? 1 : 0;
+  c->general = (p->geom != 0 || (p->use_ref && !ref_z_only) || p->metric_form == 1) ? 1 : 0;
   if (tn.force_general) c->general = 1;
   if (tn.kernel) c->variant = tn.kernel;
   if (c->general) c->variant = 2;
+  // HLLC is implemented in the thread-per-node kernels; so is the Richardson factor at the orders whose flat gradient
+  // kernel is the trace-buffer one (N <= 3)
+  if (p->riemann != 0 || (p->richardson && Nq <= 4)) c->variant = 2;
 
   auto bail = [&](int code) { free_ctx(c); return code; };
 #define CM_CUDA_B(call)                                                                                   \
@@ -495,11 +650,15 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
     if (L % tn.row_len != 0) { fail(CM_DG_EINVAL, "cm_dg_setup_tuned: row_len must divide the x-chunk length"); return bail(CM_DG_EINVAL); }
     kp.gS = tn.row_len;
   }
-  if ((int64_t)PY * L > 2147483647LL || p->ne[2] > 65535 || (int64_t)kp.gNXC * kp.gNYP > 65535) {
+  if (c->variant != 2 && ((int64_t)PY * L > 2147483647LL || p->ne[2] > 65535 || (int64_t)kp.gNXC * kp.gNYP > 65535)) {   // 3-D grid of the flat kernels
     fail(CM_DG_EINVAL, "cm_dg_setup: mesh exceeds the launch-grid limits (Ez and (Ex/L)*(Ey/PY) must be <= 65535)");
     return bail(CM_DG_EINVAL);
   }
-  kp.Ne = (int)Ne; kp.stride = c->stride; kp.sgs = p->sgs ? 1 : 0; kp.use_ref = p->use_ref ? 1 : 0;
+  kp.Ne = (int)Ne; kp.stride = c->stride; kp.sgs = p->sgs; kp.use_ref = p->use_ref ? 1 : 0;
+  kp.richardson = p->richardson; kp.riemann = p->riemann;
+  kp.cs2 = p->C_s * p->C_s;
+  for (int d = 0; d < 3; ++d) { kp.d2[d] = (c->h[d] / c->N) * (c->h[d] / c->N); kp.urelax[d] = p->u_relax[d]; }
+  kp.th.p_0 = c->prm.p_0; kp.th.kap_pd = p->R_d / (p->c_vd + p->R_d); kp.th.iRd = 1.0 / p->R_d;
   kp.th.R_d = p->R_d; kp.th.c_vd = p->c_vd; kp.th.a = p->R_v - p->R_d; kp.th.b = p->c_vv - p->c_vd;
   kp.th.T_0 = p->T_0; kp.th.I_v0 = p->I_v0; kp.th.grav = p->grav;
   kp.th.dk = kp.th.a * p->c_vd - p->R_d * kp.th.b;
@@ -528,6 +687,10 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
         double* t = &zt[(size_t)(ez * Nq + k) * CM_ZTAB_W];
         const double z = p->lo[2] + (ez + 0.5 * (c->xi[k] + 1.0)) * c->h[2];
         t[0] = p->grav * z;
+        t[7] = 0.0;                                                        // Rayleigh sponge coefficient tau_s(z) (A5, R18)
+        if (c->prm.sponge_alpha > 0.0 && z > c->prm.sponge_zs)
+          t[7] = c->prm.sponge_alpha *
+                 std::pow(std::sin(0.5 * 3.14159265358979323846 * (z - c->prm.sponge_zs) / (p->hi[2] - c->prm.sponge_zs)), (double)c->prm.sponge_gamma);
         if (p->use_ref) {
           const size_t id = ((size_t)ez * nh) * Np + (size_t)k * Nq * Nq;
           t[1] = p->ref_rho[id]; t[2] = p->ref_rhoe[id]; t[3] = c->moist ? p->ref_rhoq[id] : 0.0;
@@ -546,11 +709,11 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
     CM_CUDA_B(cudaMalloc(&d_chk, (size_t)Ne * 3 * sizeof(double)));
     GeoArgs ga = geo_args(c);
     const int thr = 128;
-    const size_t sm = (size_t)(12 * Np + 4 * thr) * sizeof(double);
-    cudaFuncSetAttribute(metrics_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    metrics_kernel<<<(unsigned)Ne, thr, sm, c->st>>>(ga, c->d_geo, d_chk);
+    const size_t sm = (size_t)(24 * Np + 4 * thr) * sizeof(double);
+    cudaError_t err = cudaFuncSetAttribute(metrics_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (err == cudaSuccess) { metrics_kernel<<<(unsigned)Ne, thr, sm, c->st>>>(ga, c->d_geo, d_chk); err = cudaGetLastError(); }
     std::vector<double> chk((size_t)Ne * 3);
-    cudaError_t err = cudaMemcpyAsync(chk.data(), d_chk, chk.size() * sizeof(double), cudaMemcpyDeviceToHost, c->st);
+    if (err == cudaSuccess) err = cudaMemcpyAsync(chk.data(), d_chk, chk.size() * sizeof(double), cudaMemcpyDeviceToHost, c->st);
     if (err == cudaSuccess) err = cudaStreamSynchronize(c->st);
     cudaFree(d_chk);
     if (err != cudaSuccess) { fail(CM_DG_ECUDA, std::string("metrics kernel: ") + cudaGetErrorString(err)); return bail(CM_DG_ECUDA); }
@@ -558,7 +721,7 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
     for (int64_t e = 0; e < Ne; ++e) { minJ = std::min(minJ, chk[3 * e]); res = std::max(res, chk[3 * e + 1]); mdx = std::min(mdx, chk[3 * e + 2]); }
     if (!(minJ > 0.0)) { fail(CM_DG_EINVAL, "cm_dg_setup: non-positive Jacobian determinant in the mesh"); return bail(CM_DG_EINVAL); }
     if (res > 1e-10) {
-      char buf[160]; std::snprintf(buf, sizeof buf, "cm_dg_setup: discrete metric identity violated (%.3e > 1e-10): fully 3-D warps are not supported", res);
+      char buf[200]; std::snprintf(buf, sizeof buf, "cm_dg_setup: discrete metric identity violated (%.3e > 1e-10): a fully 3-D warp needs metric_form = 1", res);
       fail(CM_DG_EINVAL, buf); return bail(CM_DG_EINVAL);
     }
     c->min_node_dx = mdx;
@@ -583,7 +746,13 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   c->em_bytes_per_field = std::max(fbytes, (size_t)Ne * slot * sizeof(double));
   if (p->sgs) CM_CUDA_B(cudaMalloc(&c->d_G, (size_t)c->ngrad * c->em_bytes_per_field));
   CM_CUDA_B(cudaMalloc(&c->d_part, (size_t)Ne * 7 * sizeof(double)));
-  // residual and ping-pong state are allocated on first use by cm_dg_lsrk_step
+  // LSRK residual and the two further state buffers of the stage ring (cm_dg_lsrk_step never allocates or synchronises)
+  {
+    const size_t sb = (size_t)c->nvar * fbytes;
+    CM_CUDA_B(cudaMalloc(&c->d_res, (size_t)c->nvar * c->em_bytes_per_field));
+    CM_CUDA_B(cudaMalloc(&c->d_Q2, sb)); CM_CUDA_B(cudaMemsetAsync(c->d_Q2, 0, sb, c->st));
+    CM_CUDA_B(cudaMalloc(&c->d_Q3, sb)); CM_CUDA_B(cudaMemsetAsync(c->d_Q3, 0, sb, c->st));
+  }
 
   switch (Nq) {
     case 3: c->launch_grad = cm_launch_gradient_nq3; c->launch_tend = cm_launch_tendency_nq3; break;
@@ -609,6 +778,7 @@ int cm_dg_layout(const cm_dg_ctx* ctx, int64_t* n_elem, int32_t* np, int64_t* fi
 
 int cm_dg_coords(cm_dg_ctx* ctx, double* xyz_dev) {
   if (!ctx || !xyz_dev) return fail(CM_DG_EINVAL, "cm_dg_coords: NULL argument");
+  { int rc_ = enter(ctx, "cm_dg_coords"); if (rc_) return rc_; }
   GeoArgs ga = geo_args(ctx);
   coords_kernel<<<(unsigned)ctx->Ne, 128, 0, ctx->st>>>(ga, xyz_dev);
   CM_CUDA(cudaGetLastError());
@@ -617,6 +787,7 @@ int cm_dg_coords(cm_dg_ctx* ctx, double* xyz_dev) {
 
 int cm_dg_metrics(cm_dg_ctx* ctx, double* Ja_dev, double* J_dev) {
   if (!ctx || !Ja_dev || !J_dev) return fail(CM_DG_EINVAL, "cm_dg_metrics: NULL argument");
+  { int rc_ = enter(ctx, "cm_dg_metrics"); if (rc_) return rc_; }
   const long long n = ctx->Ne * ctx->Np;
   const int thr = 256; const unsigned blocks = (unsigned)((n + thr - 1) / thr);
   if (ctx->general)
@@ -629,6 +800,7 @@ int cm_dg_metrics(cm_dg_ctx* ctx, double* Ja_dev, double* J_dev) {
 
 int cm_dg_gradient(cm_dg_ctx* ctx, const double* Q_dev, double* G_dev) {
   if (!ctx || !Q_dev || !G_dev) return fail(CM_DG_EINVAL, "cm_dg_gradient: NULL argument");
+  { int rc_ = enter(ctx, "cm_dg_gradient"); if (rc_) return rc_; }
   return run_gradient(ctx, Q_dev, G_dev, 1);
 }
 
@@ -636,32 +808,60 @@ int cm_dg_rhs(cm_dg_ctx* ctx, const double* Q_dev, double* dQ_dev, double t) {
   (void)t;   // no time-dependent forcing on this path (reading R14)
   if (!ctx || !Q_dev || !dQ_dev) return fail(CM_DG_EINVAL, "cm_dg_rhs: NULL argument");
   if (Q_dev == dQ_dev) return fail(CM_DG_EINVAL, "cm_dg_rhs: Q and dQ must be distinct buffers");
+  { int rc_ = enter(ctx, "cm_dg_rhs"); if (rc_) return rc_; }
   if (ctx->prm.sgs) { int rc = run_gradient(ctx, Q_dev, ctx->d_G, 0); if (rc) return rc; }
   return run_tendency(ctx, Q_dev, dQ_dev, nullptr, 0, 0.0, 0.0, 0.0);
 }
 
-int cm_dg_lsrk_step(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t nsteps) {
-  (void)t;
-  if (!ctx || !Q_dev) return fail(CM_DG_EINVAL, "cm_dg_lsrk_step: NULL argument");
-  if (nsteps < 0) return fail(CM_DG_EINVAL, "cm_dg_lsrk_step: nsteps must be >= 0");
-  const size_t bytes = (size_t)ctx->nvar * ctx->stride * sizeof(double);
-  if (!ctx->d_res) CM_CUDA(cudaMalloc(&ctx->d_res, (size_t)ctx->nvar * ctx->em_bytes_per_field));
-  if (!ctx->d_Q2) { CM_CUDA(cudaMalloc(&ctx->d_Q2, bytes)); CM_CUDA(cudaMemsetAsync(ctx->d_Q2, 0, bytes, ctx->st)); }
-  if (!ctx->d_Q3) { CM_CUDA(cudaMalloc(&ctx->d_Q3, bytes)); CM_CUDA(cudaMemsetAsync(ctx->d_Q3, 0, bytes, ctx->st)); }
-  // A stage never updates in place (neighbours still read the old state).  Three buffers in the cycle
-  // Q_dev -> Q2 -> Q3 -> Q2 -> Q3 -> Q_dev bring every step's five stages back into the caller's array: no copy.
-  double* const ring[6] = {Q_dev, ctx->d_Q2, ctx->d_Q3, ctx->d_Q2, ctx->d_Q3, Q_dev};
-  for (int s = 0; s < nsteps; ++s)
-    for (int st = 0; st < 5; ++st) {
-      if (ctx->prm.sgs) { int rc = run_gradient(ctx, ring[st], ctx->d_G, 0); if (rc) return rc; }
-      int rc = run_tendency(ctx, ring[st], ctx->d_res, ring[st + 1], 1, kRKA[st], kRKB[st], dt);
-      if (rc) return rc;
-    }
+int cm_dg_filter(cm_dg_ctx* ctx, double* Q_dev) {
+  if (!ctx || !Q_dev) return fail(CM_DG_EINVAL, "cm_dg_filter: NULL argument");
+  if (ctx->prm.filter_order <= 0) return fail(CM_DG_ESTATE, "cm_dg_filter: the ctx was set up with filter_order = 0");
+  int rc = enter(ctx, "cm_dg_filter"); if (rc) return rc;
+  FilterArgs a;
+  a.Nq = ctx->Nq; a.Np = ctx->Np; a.nvar = ctx->nvar; a.general = ctx->general; a.use_ref = ctx->prm.use_ref;
+  a.stride = ctx->stride; a.Q = Q_dev; a.erow = ctx->d_erow; a.ztab = ctx->d_ztab; a.ref = ctx->d_ref;
+  for (int i = 0; i < CM_MAXNQ; ++i) for (int j = 0; j < CM_MAXNQ; ++j) a.F[i][j] = ctx->Filt[i][j];
+  {
+    Timed tm(ctx, 2);
+    filter_kernel<<<(unsigned)ctx->Ne, 128, 2 * ctx->Np * sizeof(double), ctx->st>>>(a);
+  }
+  CM_CUDA(cudaGetLastError());
   return CM_DG_OK;
+}
+
+int cm_dg_lsrk_step_table(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t nsteps, int32_t nstages,
+                          const double* A, const double* B, const double* C) {
+  (void)t; (void)C;   // no time-dependent forcing on this path (reading R14)
+  if (!ctx || !Q_dev || !A || !B) return fail(CM_DG_EINVAL, "cm_dg_lsrk_step_table: NULL argument");
+  if (nsteps < 0 || nstages < 1) return fail(CM_DG_EINVAL, "cm_dg_lsrk_step_table: nsteps must be >= 0 and nstages >= 1");
+  if (A[0] != 0.0) return fail(CM_DG_EINVAL, "cm_dg_lsrk_step_table: A[0] must be 0 (the residual starts from zero)");
+  int rc = enter(ctx, "cm_dg_lsrk_step_table"); if (rc) return rc;
+  const size_t bytes = (size_t)ctx->nvar * ctx->stride * sizeof(double);
+  // A stage never updates in place (neighbours still read the old state).  The stages cycle
+  // Q_dev -> Q2 -> Q3 -> Q2 -> ... -> Q_dev: the last stage of a step writes the caller's array, no copy is appended
+  // (a one-stage scheme writes Q2 and is copied back).
+  for (int s = 0; s < nsteps; ++s) {
+    double* src = Q_dev;
+    for (int st = 0; st < nstages; ++st) {
+      double* dst = (st == nstages - 1 && nstages > 1) ? Q_dev : ((st & 1) ? ctx->d_Q3 : ctx->d_Q2);
+      if (ctx->prm.sgs) { rc = run_gradient(ctx, src, ctx->d_G, 0); if (rc) return rc; }
+      rc = run_tendency(ctx, src, ctx->d_res, dst, 1, A[st], B[st], dt);
+      if (rc) return rc;
+      src = dst;
+    }
+    if (nstages == 1) CM_CUDA(cudaMemcpyAsync(Q_dev, ctx->d_Q2, bytes, cudaMemcpyDeviceToDevice, ctx->st));
+    if (ctx->prm.filter_order > 0) { rc = cm_dg_filter(ctx, Q_dev); if (rc) return rc; }
+  }
+  return CM_DG_OK;
+}
+
+int cm_dg_lsrk_step(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t nsteps) {
+  return cm_dg_lsrk_step_table(ctx, Q_dev, t, dt, nsteps, 5, kRKA, kRKB, nullptr);
 }
 
 int cm_dg_diagnostics(cm_dg_ctx* ctx, const double* Q_dev, cm_dg_diag* out) {
   if (!ctx || !Q_dev || !out) return fail(CM_DG_EINVAL, "cm_dg_diagnostics: NULL argument");
+  { int rc_ = enter(ctx, "cm_dg_diagnostics"); if (rc_) return rc_; }
   DiagArgs a;
   a.Nq = ctx->Nq; a.Np = ctx->Np; a.nvar = ctx->nvar; a.general = ctx->general; a.use_ref = ctx->prm.use_ref;
   a.Ne = ctx->Ne; a.stride = ctx->stride; a.Q = Q_dev; a.geo = ctx->d_geo; a.erow = ctx->d_erow; a.ztab = ctx->d_ztab;
@@ -691,6 +891,7 @@ static int stage_buffer(cm_dg_ctx* ctx, size_t bytes) {
 
 int cm_dg_rhs_host(cm_dg_ctx* ctx, const double* Q_host, double* dQ_host, double t) {
   if (!ctx || !Q_host || !dQ_host) return fail(CM_DG_EINVAL, "cm_dg_rhs_host: NULL argument");
+  { int rc_ = enter(ctx, "cm_dg_rhs_host"); if (rc_) return rc_; }
   const size_t bytes = (size_t)ctx->nvar * ctx->stride * sizeof(double);
   int rc = stage_buffer(ctx, bytes); if (rc) return rc;
   double* dq = ctx->d_stage; double* dd = ctx->d_stage + (size_t)ctx->nvar * ctx->stride;
@@ -703,6 +904,7 @@ int cm_dg_rhs_host(cm_dg_ctx* ctx, const double* Q_host, double* dQ_host, double
 
 int cm_dg_lsrk_step_host(cm_dg_ctx* ctx, double* Q_host, double t, double dt, int32_t nsteps) {
   if (!ctx || !Q_host) return fail(CM_DG_EINVAL, "cm_dg_lsrk_step_host: NULL argument");
+  { int rc_ = enter(ctx, "cm_dg_lsrk_step_host"); if (rc_) return rc_; }
   const size_t bytes = (size_t)ctx->nvar * ctx->stride * sizeof(double);
   int rc = stage_buffer(ctx, bytes); if (rc) return rc;
   double* dq = ctx->d_stage;

@@ -35,7 +35,7 @@ __device__ __forceinline__ double cm_sqrt(double a) {
   return (a > 0.0) ? r : 0.0;
 }
 
-struct CmSite { double Phi, rho_r, rhoe_r, rhoq_r, E_r, q_r, icvm_r; };
+struct CmSite { double Phi, rho_r, rhoe_r, rhoq_r, E_r, q_r, icvm_r, taus /* Rayleigh sponge coefficient (A5) */; };
 struct CmPrim { double rho, ir, u, v, w, q, K, p, pp, h, c2, drho; };
 
 // geopotential + reference state at node n (k = its zeta index) of element e
@@ -44,10 +44,11 @@ __device__ __forceinline__ void cm_load_site(const CmKP& p, int e, int n, int k,
   if constexpr (GEOM == 0) {
     const double2* t = reinterpret_cast<const double2*>(p.ztab + (size_t)(__ldg(p.erow + e) + k) * CM_ZTAB_W);
     double2 a = __ldg(t), b = __ldg(t + 1), c = __ldg(t + 2), d = __ldg(t + 3);
-    s.Phi = a.x; s.rho_r = a.y; s.rhoe_r = b.x; s.rhoq_r = b.y; s.E_r = c.x; s.q_r = c.y; s.icvm_r = d.x;
+    s.Phi = a.x; s.rho_r = a.y; s.rhoe_r = b.x; s.rhoq_r = b.y; s.E_r = c.x; s.q_r = c.y; s.icvm_r = d.x; s.taus = d.y;
   } else {
     const size_t idx = (size_t)e * CmNodes<Nq>::NP + n;
     s.Phi = p.th.grav * __ldg(p.geo + 10 * p.stride + idx);
+    s.taus = __ldg(p.geo + 15 * p.stride + idx);
     if (p.use_ref) {
       s.rho_r = __ldg(p.ref + idx);
       s.rhoe_r = __ldg(p.ref + p.stride + idx);
@@ -130,6 +131,95 @@ __device__ __forceinline__ void cm_flux_axis(const double* Y, const CmPrim& P, b
   Fn[3] = s * (Y[3] * wA + ((AX == 2) ? P.pp : 0.0) + Y[0] * tA2);
   Fn[4] = s * ((Y[4] + P.p) * ud + Y[0] * eA);
   if (MOIST) Fn[5] = s * (Y[5] * ud + Y[0] * dqA);
+}
+
+// virtual potential temperature without condensate (eq. 40, reading R25) from pressure and 1 / rho
+__device__ __forceinline__ double cm_theta_v(const CmThermo& th, double pr, double ir) {
+  return pr * ir * th.iRd * pow(th.p_0 / pr, th.kap_pd);
+}
+
+// O5 / O11: eddy viscosity and packed SGS fluxes of one node.  Gr[s][c] = d s / d x_c for s = u, v, w, h_tot, q_t;
+// thv, dthv_dz = theta_v and its vertical derivative (used when p.richardson); cs2d2 = (C_s Delta)^2 of eq. (38);
+// d2 = squared mixing lengths of eq. (39c).  out = tau xx,yy,zz,xy,xz,yz | J + D x,y,z | d_q x,y,z  (eq. 34-37).
+template <bool MOIST>
+__device__ __forceinline__ void cm_closure(const CmKP& p, const double (&Gr)[5][3], double cs2d2, double d2x, double d2y,
+                                           double d2z, double thv, double dthv_dz, double (&out)[12]) {
+  const double Sxx = Gr[0][0], Syy = Gr[1][1], Szz = Gr[2][2];
+  const double Sxy = 0.5 * (Gr[0][1] + Gr[1][0]), Sxz = 0.5 * (Gr[0][2] + Gr[2][0]), Syz = 0.5 * (Gr[1][2] + Gr[2][1]);
+  const double ss2 = Sxx * Sxx + Syy * Syy + Szz * Szz + 2.0 * (Sxy * Sxy + Sxz * Sxz + Syz * Syz);   // S_ij S_ij
+  double nu;
+  if (p.sgs == 2) {
+    // Vreman (eq. 39a-d): beta_ij = Delta_m^2 u_i,m u_j,m; B = second invariant of beta
+    double b[3][3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int j = i; j < 3; ++j) b[i][j] = d2x * Gr[i][0] * Gr[j][0] + d2y * Gr[i][1] * Gr[j][1] + d2z * Gr[i][2] * Gr[j][2];
+    const double B = b[0][0] * b[1][1] + b[0][0] * b[2][2] + b[1][1] * b[2][2] - (b[0][2] * b[0][2] + b[0][1] * b[0][1] + b[1][2] * b[1][2]);
+    double aa = 0.0;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int j = 0; j < 3; ++j) aa += Gr[i][j] * Gr[i][j];
+    nu = (aa > 0.0 && B > 0.0) ? 2.5 * p.cs2 * sqrt(B / aa) : 0.0;
+  } else {
+    nu = cs2d2 * cm_sqrt(2.0 * ss2);                                       // eq. (38)
+  }
+  if (p.richardson) {
+    // eq. (40): Ri = (g / theta_v) (d theta_v / dz) / |S|^2, |S|^2 = 2 S_ij S_ij; f_b = max(0, 1 - Ri / Pr_t)^(1/4)
+    const double N2 = (p.th.grav / thv) * dthv_dz;
+    double fb = 1.0;
+    if (N2 > 0.0) {
+      const double t = 1.0 - (N2 / (2.0 * ss2)) * p.inv_Pr;
+      fb = (t > 0.0) ? sqrt(sqrt(t)) : 0.0;
+    }
+    nu *= fb;
+  }
+  const double m2nu = -2.0 * nu, mDt = -nu * p.inv_Pr;
+  out[0] = m2nu * Sxx; out[1] = m2nu * Syy; out[2] = m2nu * Szz; out[3] = m2nu * Sxy; out[4] = m2nu * Sxz; out[5] = m2nu * Syz;
+  out[6] = mDt * Gr[3][0]; out[7] = mDt * Gr[3][1]; out[8] = mDt * Gr[3][2];
+  out[9] = MOIST ? mDt * Gr[4][0] : 0.0; out[10] = MOIST ? mDt * Gr[4][1] : 0.0; out[11] = MOIST ? mDt * Gr[4][2] : 0.0;
+}
+
+// A . F1(Y) for all variables (first-order flux only; A = sJ n)
+template <bool MOIST>
+__device__ __forceinline__ void cm_flux1_dir(const double* Y, const CmPrim& P, double A0, double A1, double A2, double* Fn) {
+  const double uA = A0 * P.u + A1 * P.v + A2 * P.w;
+  Fn[0] = Y[0] * uA;
+  Fn[1] = Y[1] * uA + P.pp * A0; Fn[2] = Y[2] * uA + P.pp * A1; Fn[3] = Y[3] * uA + P.pp * A2;
+  Fn[4] = (Y[4] + P.p) * uA;
+  if (MOIST) Fn[5] = Y[5] * uA;
+}
+
+// HLLC flux (Toro, Spruce & Speares 1994): Fs = sJ n.F1* from the two states, A = sJ n, AFm / AFp = A.F1 of the
+// two sides.  Wave speeds S_L = min(u_L - c_L, u_R - c_R), S_R = max(u_L + c_L, u_R + c_R); p' in the momentum
+// flux, full p in the energy relation (same reading as the oracle).
+template <bool MOIST>
+__device__ __forceinline__ void cm_hllc(const double* Ym, const CmPrim& Pm, const double* AFm, const double* Yp, const CmPrim& Pp,
+                                        const double* AFp, const double* A, double sJ, double* Fs) {
+  constexpr int NV = MOIST ? 6 : 5;
+  const double isJ = 1.0 / sJ;
+  const double n0 = A[0] * isJ, n1 = A[1] * isJ, n2 = A[2] * isJ;
+  const double unm = Pm.u * n0 + Pm.v * n1 + Pm.w * n2, unp = Pp.u * n0 + Pp.v * n1 + Pp.w * n2;
+  const double cm_ = sqrt(Pm.c2), cp = sqrt(Pp.c2);
+  const double SL = fmin(unm - cm_, unp - cp), SR = fmax(unm + cm_, unp + cp);
+  if (SL >= 0.0) { for (int v = 0; v < NV; ++v) Fs[v] = AFm[v]; return; }
+  if (SR <= 0.0) { for (int v = 0; v < NV; ++v) Fs[v] = AFp[v]; return; }
+  const double Sstar = ((Pp.pp - Pm.pp) + Ym[0] * unm * (SL - unm) - Yp[0] * unp * (SR - unp)) /
+                       (Ym[0] * (SL - unm) - Yp[0] * (SR - unp));
+  const bool left = Sstar >= 0.0;
+  const double* Y = left ? Ym : Yp; const CmPrim& P = left ? Pm : Pp;
+  const double un = left ? unm : unp, SK = left ? SL : SR;
+  const double* AF = left ? AFm : AFp;
+  // the jump U*_K - U_K formed analytically (rho* - rho = rho (S* - u_n) / (S_K - S*)): no cancellation of O(rho c) terms
+  const double ds = Sstar - un;
+  const double rs = Y[0] * (SK - un) / (SK - Sstar), drho = Y[0] * ds / (SK - Sstar);
+  double dU[6];
+  dU[0] = drho;
+  dU[1] = drho * P.u + rs * ds * n0; dU[2] = drho * P.v + rs * ds * n1; dU[3] = drho * P.w + rs * ds * n2;
+  dU[4] = drho * (Y[4] / Y[0]) + rs * ds * (Sstar + P.p / (Y[0] * (SK - un)));
+  if (MOIST) dU[5] = drho * P.q;
+  for (int v = 0; v < NV; ++v) Fs[v] = AF[v] + sJ * (SK * dU[v]);
 }
 
 template <int NV>

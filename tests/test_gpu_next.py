@@ -1,0 +1,153 @@
+"""GPU parity of the NEXT rows (Vreman / Richardson, sponge, element filter, LSRK tables, HLLC, curl-invariant metrics)
+against the oracle functions that tests/test_oracle_next.py pins, through the C ABI, element by element."""
+import numpy as np
+import pytest
+
+import workloads as W
+from parity_util import RHS_TOL, STEP_TOL, rhs_errors, small_config, state_errors
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2110_00853_b200 as pkg
+    return pkg
+
+
+def _rhs_check(P, oracle_mod, cfg, Q, dt, steps=3, tuning=None):
+    o = oracle_mod.Oracle(cfg); g = P.CmDg(cfg, tuning=tuning)
+    Qs = o.lsrk54(Q, dt, steps)                      # a state with flow: every closure term is active
+    err = rhs_errors(g.to_host(g.rhs(g.to_device(Qs))), o.rhs(Qs), cfg, Qs, o.diagnostics(Qs)["min_node_dx"])
+    g.close()
+    return err
+
+
+@pytest.mark.parametrize("k,N", [(2, 4), (3, 4), (4, 4), (5, 4), (5, 3), (5, 5)])
+@pytest.mark.parametrize("sgs,rich", [(2, 0), (1, 1), (2, 1)])
+def test_vreman_and_richardson_rhs_parity(P, oracle_mod, k, N, sgs, rich):
+    cfg, Q, dt = small_config(k, N=N)
+    cfg = dict(cfg, sgs=sgs, richardson=rich)
+    # config 2 starts at rest: after a few steps the velocity gradients are ~1e-6 1/s and sqrt(B / u_ij u_ij), f_b are
+    # evaluated on round-off; the bubble has to be moving for the closure to be a meaningful input
+    err = _rhs_check(P, oracle_mod, cfg, Q, dt, steps=60 if k == 2 else 3)
+    assert np.all(err <= RHS_TOL), err
+
+
+@pytest.mark.parametrize("tuning", [{"kernel": 7}, {"kernel": 2}])
+def test_vreman_richardson_other_kernels(P, oracle_mod, tuning):
+    cfg, Q, dt = small_config(5)
+    cfg = dict(cfg, sgs=2, richardson=1)
+    err = _rhs_check(P, oracle_mod, cfg, Q, dt, tuning=tuning)
+    assert np.all(err <= RHS_TOL), err
+
+
+def test_vreman_steps(P, oracle_mod):
+    cfg, Q, dt = small_config(5)
+    cfg = dict(cfg, sgs=2, richardson=1)
+    o = oracle_mod.Oracle(cfg); g = P.CmDg(cfg)
+    Qd = g.to_device(Q); g.lsrk_step(Qd, dt, 20)
+    err = state_errors(g.to_host(Qd), o.lsrk54(Q, dt, 20))
+    assert np.all(err <= STEP_TOL), err
+
+
+@pytest.mark.parametrize("k", [2, 4])
+def test_sponge_rhs_parity(P, oracle_mod, k):
+    cfg, Q, dt = small_config(k)
+    cfg = dict(cfg, sponge_alpha=0.4, sponge_zs=0.55 * cfg["hi"][2], sponge_gamma=2, u_relax=(10.0, 0.0, 0.0))
+    err = _rhs_check(P, oracle_mod, cfg, Q, dt)
+    assert np.all(err <= RHS_TOL), err
+    o = oracle_mod.Oracle(cfg); g = P.CmDg(cfg)
+    Qd = g.to_device(Q); g.lsrk_step(Qd, dt, 30)
+    assert np.all(state_errors(g.to_host(Qd), o.lsrk54(Q, dt, 30)) <= STEP_TOL)
+
+
+@pytest.mark.parametrize("k", [1, 4, 5])
+def test_filter_parity(P, oracle_mod, k):
+    cfg, Q, dt = small_config(k)
+    cfg = dict(cfg, filter_order=64)
+    o = oracle_mod.Oracle(cfg); g = P.CmDg(cfg)
+    Qf = g.to_host(g.filter(g.to_device(Q)))
+    Qo = o.filter(Q)
+    for v in range(cfg["nvar"]):
+        assert np.max(np.abs(Qf[..., v] - Qo[..., v])) <= 1e-13 * np.max(np.abs(Qo[..., v])), v
+    assert np.max(np.abs(Qo - Q)) > 0
+    Qd = g.to_device(Q); g.lsrk_step(Qd, dt, 20)       # the filter follows every step
+    assert np.all(state_errors(g.to_host(Qd), o.lsrk54(Q, dt, 20)) <= STEP_TOL)
+    with pytest.raises(P.CmDgError):
+        g0 = P.CmDg(small_config(k)[0]); g0.filter(g0.to_device(Q))
+
+
+@pytest.mark.parametrize("k", [1, 5])
+def test_lsrk_table_parity(P, oracle_mod, k):
+    cfg, Q, dt = small_config(k)
+    o = oracle_mod.Oracle(cfg); g = P.CmDg(cfg)
+    A3, B3 = [0.0, -5.0 / 9.0, -153.0 / 128.0], [1.0 / 3.0, 15.0 / 16.0, 8.0 / 15.0]    # Williamson (3,3)
+    for A, B, n in ((A3, B3, 15), ([0.0], [1.0], 7), ([0.0, -0.5], [0.5, 1.0], 6)):
+        Qd = g.to_device(Q); g.lsrk_step_table(Qd, 0.3 * dt, n, A, B)
+        err = state_errors(g.to_host(Qd), o.lsrk_table(Q, 0.3 * dt, n, A, B))
+        assert np.all(err <= STEP_TOL), (A, err)
+    A5, B5, _ = oracle_mod.lsrk54_coeffs()
+    Qa = g.to_device(Q); g.lsrk_step_table(Qa, dt, 4, A5, B5)
+    Qb = g.to_device(Q); g.lsrk_step(Qb, dt, 4)
+    assert bool((Qa == Qb).all())
+    with pytest.raises(P.CmDgError):
+        g.lsrk_step_table(Qa, dt, 1, [0.5], [1.0])
+
+
+@pytest.mark.parametrize("k", [1, 3, 4, 5])
+def test_hllc_parity(P, oracle_mod, k):
+    cfg, Q, dt = small_config(k)
+    cfg = dict(cfg, riemann=1)
+    err = _rhs_check(P, oracle_mod, cfg, Q, dt)
+    assert np.all(err <= RHS_TOL), err
+    o = oracle_mod.Oracle(cfg); g = P.CmDg(cfg)
+    Qd = g.to_device(Q); g.lsrk_step(Qd, dt, 20)
+    assert np.all(state_errors(g.to_host(Qd), o.lsrk54(Q, dt, 20)) <= STEP_TOL)
+
+
+def test_curl_invariant_metrics_parity_and_free_stream(P, oracle_mod):
+    from test_oracle_next import warped_3d
+    cfg, Y = warped_3d(metric_form=1, sgs=1)
+    o = oracle_mod.Oracle(cfg); g = P.CmDg(cfg)
+    Ja, J = g.metrics(); Ja = g.to_host(Ja); J = g.to_host(J)[..., 0]
+    for e in range(0, o.Ne, 5):
+        go = o.elem_geometry(e)
+        assert np.max(np.abs(Ja[e].reshape(-1, 3, 3) - go["Ja"])) <= 1e-12 * np.max(np.abs(go["Ja"]))
+        assert np.max(np.abs(J[e] - go["J"])) <= 1e-12 * np.max(go["J"])
+    one = np.ones(Y.shape[:2])
+    Qu = W.conserved(cfg, 1.1 * one, 12.0 * one, -7.0 * one, 3.0 * one, 288.0 * one, 0 * one, 0 * one)
+    dQ = g.to_host(g.rhs(g.to_device(Qu)))
+    dx = g.diagnostics(g.to_device(Qu))["min_node_dx"]
+    Tf = np.array([13.2, 1.1 * 144 + 1e5, 1.1 * 144 + 1e5, 1.1 * 144 + 1e5, 3.6e5 * 12]) / dx
+    for v in range(5):
+        assert np.max(np.abs(dQ[..., v])) <= 1e-13 * Tf[v], v
+    rng = np.random.default_rng(W.SEED0 + 31)
+    shp = Y.shape[:2]
+    Q = W.conserved(cfg, 1.1 + 1e-3 * rng.uniform(-1, 1, shp), *(rng.normal(0, 2.0, shp) for _ in range(3)),
+                    295.0 + 0.1 * rng.normal(0, 1, shp), 0 * one, 0 * one)
+    err = rhs_errors(g.to_host(g.rhs(g.to_device(Q))), o.rhs(Q), cfg, Q, dx)
+    assert np.all(err <= RHS_TOL), err
+    with pytest.raises(P.CmDgError):                    # the cross-product form must still be refused on this mesh
+        P.CmDg(dict(cfg, metric_form=0))
+
+
+def test_two_contexts_interleaved_and_foreign_device(P, oracle_mod):
+    """Two ctxs of different order on one device, calls interleaved: per-ctx state only."""
+    import torch
+    c1, Q1, dt1 = small_config(5, N=4); c2, Q2, dt2 = small_config(3, N=5)
+    g1, g2 = P.CmDg(c1), P.CmDg(c2)
+    o1, o2 = oracle_mod.Oracle(c1), oracle_mod.Oracle(c2)
+    d1, d2 = g1.to_device(Q1), g2.to_device(Q2)
+    for _ in range(3):
+        g1.lsrk_step(d1, dt1, 1); g2.lsrk_step(d2, dt2, 1)
+    r1 = g1.rhs(d1); r2 = g2.rhs(d2)
+    assert np.all(state_errors(g1.to_host(d1), o1.lsrk54(Q1, dt1, 3)) <= STEP_TOL)
+    assert np.all(state_errors(g2.to_host(d2), o2.lsrk54(Q2, dt2, 3)) <= STEP_TOL)
+    assert torch.isfinite(r1).all() and torch.isfinite(r2).all()
+    if torch.cuda.device_count() > 1:
+        with torch.cuda.device(1):
+            with pytest.raises(P.CmDgError):
+                g1.rhs(d1)
