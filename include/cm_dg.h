@@ -79,7 +79,7 @@ typedef struct {
 } cm_dg_params;
 
 /* Optional scheduling knobs (HOST, copied by cm_dg_setup_tuned).  They never change what is computed (the parity tests
- * run every setting against the oracle), only how the work is laid out on the GPU.  All-zero = the defaults, except
+ * run every setting against the CPU reference of tests/), only how the work is laid out on the GPU.  All-zero = the defaults, except
  * ahead_t / ahead_g whose default is -1. */
 typedef struct {
   int32_t order_lex;     /* 1: lexicographic element order instead of the tiled one (lex_of_elem becomes the identity)   */

@@ -193,7 +193,7 @@ __device__ __forceinline__ void cm_flux1_dir(const double* Y, const CmPrim& P, d
 
 // HLLC flux (Toro, Spruce & Speares 1994): Fs = sJ n.F1* from the two states, A = sJ n, AFm / AFp = A.F1 of the
 // two sides.  Wave speeds S_L = min(u_L - c_L, u_R - c_R), S_R = max(u_L + c_L, u_R + c_R); p' in the momentum
-// flux, full p in the energy relation (same reading as the oracle).
+// flux, full p in the energy relation (reading R27 of DESIGN.md).
 template <bool MOIST>
 __device__ __forceinline__ void cm_hllc(const double* Ym, const CmPrim& Pm, const double* AFm, const double* Yp, const CmPrim& Pp,
                                         const double* AFp, const double* A, double sJ, double* Fs) {
