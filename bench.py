@@ -44,13 +44,52 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic():
-    """dram bytes per launch of the dominant kernel from the committed ncu capture, if one is recorded."""
+def kernel_source_hash():
+    """sha256 over the CUDA sources: ties a recorded ncu figure to the kernels it was captured on."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2110_00853_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        with open(os.path.join(d, f), "rb") as fh:
+            h.update(f.encode()); h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(order, ne):
+    """dram bytes per launch of the dominant kernel from the committed ncu capture -- only if that capture was taken on
+    the kernels of this tree (source hash) and on this workload; otherwise None."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(path):
-        with open(path) as f:
-            return json.load(f).get("tendency_dram_bytes_per_launch")
-    return None
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        t = json.load(f)
+    if t.get("source_hash") != kernel_source_hash() or t.get("order") != order or list(t.get("ne", [])) != list(ne):
+        return None
+    return t.get("tendency_dram_bytes_per_launch")
+
+
+def record_traffic(args):
+    """--record-traffic RAW.csv: reads dram__bytes_read.sum + dram__bytes_write.sum of the tendency kernel from an
+    `ncu -i <rep> --page raw --csv` export and stores them with the source hash and the workload."""
+    import csv
+    rows = list(csv.reader(open(args.record_traffic)))
+    hdr, units = rows[0], rows[1]
+    best = None
+    for r in rows[2:]:
+        d = dict(zip(hdr, r))
+        if "tendency" not in d.get("Kernel Name", ""):
+            continue
+        tot = 0.0
+        for k in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            u = units[hdr.index(k)]
+            tot += float(d[k]) * {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}[u]
+        best = (d["Kernel Name"], tot)
+    assert best, "no tendency kernel in " + args.record_traffic
+    out = {"tendency_dram_bytes_per_launch": best[1], "kernel": best[0], "source_hash": kernel_source_hash(),
+           "order": args.order, "ne": list(args.ne), "source": os.path.basename(args.record_traffic)}
+    with open(os.path.join(ROOT, "profiles", "traffic.json"), "w") as f:
+        json.dump(out, f, indent=1)
+    print(json.dumps(out))
 
 
 class ClockSampler:
@@ -118,6 +157,62 @@ def time_oracle(sample_ne, order, steps, warmup=0):
     return nodes * 5 * steps / el, om.num_threads(), desc, el / steps
 
 
+def cpu_info():
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    model = line.split(":", 1)[1].strip(); break
+    except OSError:
+        pass
+    return model, os.cpu_count()
+
+
+def set_oracle_threads(n):
+    """OpenMP thread count of the oracle library (libgomp's own entry point; the oracle is not modified for timing)."""
+    import ctypes
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except OSError:
+        return False
+
+
+def time_oracle_stage(cfg, Q, dt, reps=3):
+    """Best of `reps` of ONE LSRK54 stage (gradient + RHS + update) of the oracle on the given config."""
+    from oracle import oracle as om
+    o = om.Oracle(cfg)
+    Qc = Q.copy(); dU = np.zeros_like(Q)
+    best = 1e300
+    for _ in range(reps):
+        t0 = time.perf_counter(); o.lsrk54_stage(Qc, dU, dt, 0); best = min(best, time.perf_counter() - t0)
+    nodes = Q.shape[0] * Q.shape[1]
+    return {"nodes": nodes, "ms_per_stage": 1e3 * best, "node_stages_per_s": nodes / best}
+
+
+def cpu_baseline(order, full_ne, ne):
+    """the oracle as it stands on the host cores -- all cores and one thread on cuts of config 5
+    (full 3 km column), one stage of each of configs 1-4 at their stated sizes; CPU model, nproc and thread counts printed."""
+    import workloads as W
+    from oracle import oracle as om
+    model, nproc = cpu_info()
+    sample = (full_ne[0] // 4, full_ne[1] // 4, full_ne[2]) if tuple(ne) == tuple(full_ne) else tuple(ne)
+    val, threads, desc, _ = time_oracle(sample, order, 3)
+    out = {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc, "cpu_model": model, "nproc": nproc}
+    small = (max(1, sample[0] // 3), max(1, sample[1] // 3), sample[2])
+    if set_oracle_threads(1):
+        v1, t1, d1, _ = time_oracle(small, order, 1)
+        out["single_thread"] = {"value": v1, "unit": UNIT, "cores": t1, "sample": d1}
+        set_oracle_threads(threads)
+    per_cfg = {}
+    for k in (1, 2, 3, 4):
+        cfg, Q, dt = W.CONFIGS[k]()
+        per_cfg["config%d" % k] = time_oracle_stage(cfg, Q, dt)
+    out["one_stage_all_cores"] = per_cfg
+    return out
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -126,14 +221,82 @@ def run_reference(args):
     full = W.SWEEP5[args.order]
     sample = (full[0] // 4, full[1] // 4, full[2])          # 1/16 of the columns, full 3 km height
     val, threads, desc, s_per_step = time_oracle(sample, args.order, args.steps, args.warmup)
+    model, nproc = cpu_info()
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * s_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": workload_config(args, sample_note="each step = one LSRK54 step on the bounded sample: " + desc),
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
+                             "cpu_model": model, "nproc": nproc},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
+
+
+# algorithmic bytes per node and LSRK stage of the extra legs (stage 1 of a step does not read the residual)
+def stage_bytes(nvar, sgs, warped25):
+    ngrad = {5: 9, 6: 12}[nvar]
+    grad = (nvar + ngrad) * 8 if sgs else 0
+    tend = (nvar + (ngrad if sgs else 0) + nvar + nvar + nvar) * 8 - nvar * 8 / 5.0
+    geo = (2 + 2 + 2 + 1) * 8 if warped25 else 0          # z_xi, z_zeta per sweep, rho_r, rhoe_r, nodal z (SURVEY: 200 B for config 4)
+    if warped25 and not sgs:
+        geo = (2 + 2 + 1) * 8
+    return grad + tend + geo
+
+
+def bench_leg(P, torch, cfg, Q, dt, steps, peak, label, bytes_per_node_stage):
+    """K LSRK54 steps of one further workload on the library stream, CUDA events; returns a small report dict."""
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        g = P.CmDg(cfg, stream=stream)
+        Qd = torch.from_numpy(g.pack(Q)).to(g.device, non_blocking=False)
+    stream.synchronize()
+    nodes = g.n_elem * g.np
+    for _ in range(3):
+        g.lsrk_step(Qd, dt, 1)
+    stream.synchronize()
+    g.profile_begin()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        g.lsrk_step(Qd, dt, 1)
+    e1.record(stream); stream.synchronize()
+    ks = g.profile_end()
+    ms = e0.elapsed_time(e1)
+    d = g.diagnostics(Qd)
+    gbs = nodes * bytes_per_node_stage * 5 * steps / (ms * 1e-3) / 1e9
+    out = {"workload": label, "nodes": nodes, "order": int(cfg["N"]), "steps": steps, "value": nodes * 5 * steps / (ms * 1e-3),
+           "unit": UNIT, "ms_per_step": ms / steps,
+           "ms_tendency": ks["ms_tendency"] / max(1, ks["launches_tendency"]),
+           "ms_gradient": ks["ms_gradient"] / max(1, ks["launches_gradient"]),
+           "algorithmic_bytes_per_node_stage": bytes_per_node_stage, "achieved_gbs": gbs, "frac_of_measured_hbm": gbs / peak,
+           "n_nonfinite": d["n_nonfinite"]}
+    g.close(); del Qd
+    torch.cuda.empty_cache()
+    return out
+
+
+def extra_legs(P, torch, args, peak):
+    """Order sweep of config 5 at ~55 M nodes (N = 3, 5, 6), dry config 3 and terrain config 4 (BASELINE size and a
+    y-extruded variant that fills the GPU): throughput and whole-stage roofline fraction of each."""
+    import workloads as W
+    out = {"sweep": [], "configs": []}
+    for N in (3, 5, 6):
+        if N == args.order:
+            continue
+        ne = W.SWEEP5[N]
+        cfg, Q, dt = W.config5(ne=ne, N=N, hi=(6000.0, 6000.0, 3000.0))
+        out["sweep"].append(bench_leg(P, torch, cfg, Q, dt, 3, peak, "config 5 at N=%d, %dx%dx%d" % ((N,) + tuple(ne)), stage_bytes(6, 1, False)))
+        del cfg, Q
+    cfg, Q, dt = W.config3()
+    out["configs"].append(bench_leg(P, torch, cfg, Q, dt, 20, peak, "config 3 (dry CBL, SL, flat) 32x32x16", stage_bytes(5, 1, False)))
+    cfg, Q, dt = W.config3(ne=(96, 96, 48), hi=(19200.0, 19200.0, 9000.0))
+    out["configs"].append(bench_leg(P, torch, cfg, Q, dt, 5, peak, "config 3 scaled to 96x96x48 elements", stage_bytes(5, 1, False)))
+    cfg, Q, dt = W.config4()
+    out["configs"].append(bench_leg(P, torch, cfg, Q, dt, 20, peak, "config 4 (mountain, inviscid, stored metrics) 120x1x30", stage_bytes(5, 0, True)))
+    cfg, Q, dt = W.config4(ne=(120, 96, 30))
+    out["configs"].append(bench_leg(P, torch, cfg, Q, dt, 5, peak, "config 4 extruded to 120x96x30 elements", stage_bytes(5, 0, True)))
+    return out
 
 
 def workload_config(args, sample_note=None):
@@ -221,7 +384,8 @@ def run_ours(args):
     d1 = g.diagnostics(Qd)
 
     # ---- RHS alone (cm_dg_rhs), same state
-    dQ = g.empty(nv)
+    with torch.cuda.stream(stream):                  # allocate (and zero-fill) on the stream the library writes on
+        dQ = g.empty(nv)
     for _ in range(3):
         g.rhs(Qd, dQ)
     e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
@@ -253,7 +417,7 @@ def run_ours(args):
     stage_bytes = nodes * (B_GRAD[nv] + (4 * B_TEND[nv] + B_TEND_STAGE1[nv]) / 5.0)
     stage_gbs = stage_bytes * 5 * K / (ms * 1e-3) / 1e9
     roof = {"bound": "hbm", "kernel": "cm_tendency_kernel (fused tendency + LSRK update)", "achieved": ach, "peak": peak,
-            "unit": "GB/s", "frac": ach / peak, "traffic": ncu_traffic(), "peak_source": peak_src,
+            "unit": "GB/s", "frac": ach / peak, "traffic": ncu_traffic(args.order, args.ne), "peak_source": peak_src,
             "algorithmic_bytes_per_launch": bytes_tend, "ms_per_launch": t_tend,
             "share_of_step": ks["ms_tendency"] / (ks["ms_tendency"] + ks["ms_gradient"] + ks["ms_other"]),
             "gradient_kernel": {"achieved": nodes * B_GRAD[nv] / (t_grad * 1e-3) / 1e9, "ms_per_launch": t_grad,
@@ -275,11 +439,12 @@ def run_ours(args):
                              "rel_energy_change": (d1["energy"] - d0["energy"]) / d0["energy"],
                              "n_nonfinite": d1["n_nonfinite"]},
             "setup_s": t_gen}
+    if rank == 0 and world == 1 and not args.no_extra:
+        g.close(); del Qd, Qh
+        torch.cuda.empty_cache()
+        line["extra"] = extra_legs(P, torch, args, peak)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        full = W.SWEEP5[args.order]
-        sample = (full[0] // 4, full[1] // 4, full[2]) if tuple(args.ne) == tuple(full) else tuple(args.ne)
-        val, threads, desc, _ = time_oracle(sample, args.order, 3)
-        line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
+        line["cpu_baseline"] = cpu_baseline(args.order, W.SWEEP5[args.order], args.ne)
     if rank == 0:
         print(json.dumps(line))
     if dist is not None:
@@ -296,6 +461,9 @@ def main():
     ap.add_argument("--ne", type=int, nargs=3, default=None, help="element counts (default: the full config-5 mesh)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--record-traffic", default=None, metavar="RAW.csv",
+                    help="store the tendency kernel's ncu DRAM bytes (ncu --page raw --csv export) in profiles/traffic.json")
+    ap.add_argument("--no-extra", action="store_true", help="skip the extra legs (order sweep, configs 3 and 4)")
     ap.add_argument("--tuning", nargs="*", default=None, metavar="KEY=VAL",
                     help="cm_dg_tuning fields for kernel experiments (e.g. kernel=7 row_len=16); default: the library's defaults")
     args = ap.parse_args()
@@ -306,7 +474,9 @@ def main():
     import workloads as W
     if args.ne is None:
         args.ne = list(W.SWEEP5[args.order])
-    if args.impl == "reference":
+    if args.record_traffic:
+        record_traffic(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
