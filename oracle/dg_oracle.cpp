@@ -19,6 +19,8 @@
 //   O12 Rayleigh sponge (eq. A4-A5) and the exponential element filter (eq. 52)
 //   O13 any 2N-storage LSRK coefficient table, HLLC flux (named P:L256; Toro et al. 1994, textbook form),
 //       curl-invariant metric terms (Kopriva 2006) for fully 3-D warps
+//   O14 surface fluxes at the bottom wall: aerodynamic drag law (eq. A2), prescribed evaporation and latent
+//       heat flux; density-weighted horizontal statistics (eq. B1-B4)
 // Readings of the paper where it is silent or garbled are R1..R29 of DESIGN.md.
 //
 // Data layout of the oracle (deliberately NOT the GPU layout): array-of-structures,
@@ -64,6 +66,9 @@ struct Ctx {
   int filter_order = 0; double filter_alpha = 36.0436533891172;   // eq. (52); alpha = -log(2^-52)
   int riemann = 0;                 // 0 Rusanov (eq. 27) | 1 HLLC
   int metric_form = 0;             // 0 cross-product (R4) | 1 curl-invariant
+  double drag_cd = 0.0;            // C_d of the drag law (A2) on the bottom wall, 0 = free slip
+  double lhf_bottom = 0.0;         // latent heat flux LHF [W m^-2] added to SHF in the wall energy flux
+  double evap_bottom = 0.0;        // evaporation E [kg m^-2 s^-1] into the domain through the bottom wall
   double xi[MAXNQ], w[MAXNQ], D[MAXNQ][MAXNQ];
   double Filt[MAXNQ][MAXNQ];       // 1-D nodal filter matrix V diag(sigma) V^-1
   // optional cache of per-element geometry (same function fills it; see elem_geo)
@@ -597,6 +602,25 @@ void rhs_element(const Ctx& c, const double* Q, int64_t e, const double* Ge, con
             Fstar[v] += a2;
           }  // wall: n.F2* = 0 (R10)
         if (en < 0 && f == 4 && c.shf_bottom != 0.0) Fstar[4] += -c.shf_bottom;  // prescribed upward energy flux
+        if (en < 0 && f == 4) {
+          // O14 (R30).  n_in = -nrm is the inward normal of App. A.  All are fluxes INTO the domain, Fstar is outward.
+          // energy: n_in . rho (J + D) = SHF + LHF; water and, with it, mass (same right-hand side):
+          // E = n_in . (rho d_qv)
+          Fstar[4] += -c.lhf_bottom;
+          if (nv == 6) { Fstar[5] += -c.evap_bottom; Fstar[0] += -c.evap_bottom; }
+          if (c.drag_cd > 0.0) {
+            // drag law (A2): n_in . (rho tau) = -rho C_d |u_p,int| u_p,int, u_p,int = wall-parallel velocity at the first
+            // layer of interior nodes of the surface-adjacent element: the node above this one in the column
+            int ni = n + Nq * Nq;
+            Prim Pi = prim_at(c, Q, e, ni, g.x[3 * ni + 2]);
+            double un = Pi.u[0] * nrm[0] + Pi.u[1] * nrm[1] + Pi.u[2] * nrm[2];
+            double up[3], mag = 0;
+            for (int i = 0; i < 3; ++i) { up[i] = Pi.u[i] - un * nrm[i]; mag += up[i] * up[i]; }
+            mag = std::sqrt(mag);
+            // momentum equation: -div(rho tau); outward normal flux nrm . (rho tau) = -n_in . (rho tau)
+            for (int i = 0; i < 3; ++i) Fstar[1 + i] += Ym[0] * c.drag_cd * mag * up[i];
+          }
+        }
         for (int v = 0; v < nv; ++v) {
           if (form == 0) {
             dQ[(size_t)n * nv + v] -= lift * Fstar[v];
@@ -717,6 +741,59 @@ void lsrk_steps(const Ctx& c, double* Q, double dt, int nsteps, int nstages, con
 
 }  // namespace
 
+// ---------------------------------------------------------------- O14: density-weighted horizontal statistics (App. B)
+// Levels: every nodal zeta-plane of every element layer, l = ez * Nq + k (the planes of an element interface appear twice,
+// once from each side: the DG solution is double-valued there).  <a>_l = sum W a / sum W over the nodes of the plane, with
+// the area element of the zeta = const surface as weight, W = w_i w_j |Ja^3| ("metric terms accounted for").
+// phi = u, v, w, h_tot, q_t, theta_v.  out[l][20] = <z>, <rho>, phibar (B1) x6, (w'phi')bar (B2) x6, (phi'^2)bar (B4) x6
+// with phi' = phi - phibar (B3), w' = w - wbar.
+constexpr int NPROF = 20;
+void favre_profiles(const Ctx& c, const double* Q, double* out) {
+  const int Nq = c.Nq, nlev = c.ne[2] * Nq;
+  std::vector<double> sumW(nlev, 0.0);
+  for (int l = 0; l < nlev * NPROF; ++l) out[l] = 0.0;
+  // pass 1: <z>, <rho>, <rho phi>
+  for (int pass = 0; pass < 2; ++pass) {
+    for (int ez = 0; ez < c.ne[2]; ++ez)
+      for (int ey = 0; ey < c.ne[1]; ++ey)
+        for (int ex = 0; ex < c.ne[0]; ++ex) {
+          int64_t e = elem_index(c, ex, ey, ez);
+          Geo g; elem_geo(c, e, g);
+          for (int n = 0; n < c.Np; ++n) {
+            int i = n % Nq, j = (n / Nq) % Nq, k = n / (Nq * Nq);
+            int l = ez * Nq + k;
+            const double* a3 = g.Ja + 9 * n + 6;
+            double W = c.w[i] * c.w[j] * std::sqrt(a3[0] * a3[0] + a3[1] * a3[1] + a3[2] * a3[2]);
+            Prim P = prim_at(c, Q, e, n, g.x[3 * n + 2]);
+            double phi[6]; grad_vars(P, phi);
+            double* o = out + (size_t)l * NPROF;
+            if (pass == 0) {
+              sumW[l] += W;
+              o[0] += W * g.x[3 * n + 2];
+              o[1] += W * P.rho;
+              for (int m = 0; m < 6; ++m) o[2 + m] += W * P.rho * phi[m];
+            } else {
+              double wp = phi[2] - o[2 + 2];
+              for (int m = 0; m < 6; ++m) {
+                double fp = phi[m] - o[2 + m];
+                o[8 + m] += W * P.rho * wp * fp;
+                o[14 + m] += W * P.rho * fp * fp;
+              }
+            }
+          }
+        }
+    for (int l = 0; l < nlev; ++l) {
+      double* o = out + (size_t)l * NPROF;
+      if (pass == 0) {
+        o[0] /= sumW[l]; o[1] /= sumW[l];                                  // <z>, <rho>
+        for (int m = 0; m < 6; ++m) o[2 + m] = (o[2 + m] / sumW[l]) / o[1];   // (B1)
+      } else {
+        for (int m = 0; m < 12; ++m) o[8 + m] = (o[8 + m] / sumW[l]) / o[1];  // (B2), (B4)
+      }
+    }
+  }
+}
+
 // ================================================================= C ABI (ctypes)
 extern "C" {
 
@@ -742,6 +819,7 @@ struct odg_params {
   int32_t filter_order; double filter_alpha;
   int32_t riemann;
   int32_t metric_form;
+  double drag_cd, lhf_bottom, evap_bottom;
 };
 
 void odg_lgl(int N, double* xi, double* w) { lgl_nodes_weights(N, xi, w); }
@@ -771,6 +849,7 @@ void* odg_create(const odg_params* p) {
   for (int d = 0; d < 3; ++d) c->u_relax[d] = p->u_relax[d];
   c->filter_order = p->filter_order; c->filter_alpha = p->filter_alpha;
   c->riemann = p->riemann; c->metric_form = p->metric_form;
+  c->drag_cd = p->drag_cd; c->lhf_bottom = p->lhf_bottom; c->evap_bottom = p->evap_bottom;
   lgl_nodes_weights(c->N, c->xi, c->w);
   deriv_matrix(c->N, c->xi, c->D);
   if (c->filter_order > 0) filter_matrix(c->N, c->xi, c->filter_order, c->filter_alpha, c->Filt);
@@ -974,6 +1053,9 @@ void odg_diagnostics(void* h, const double* Q, double* out) {
   }
   out[0] = mass; out[1] = energy; out[2] = water; out[3] = ke / vol; out[4] = wmax; out[5] = dxmin; out[6] = vol; out[7] = nonf;
 }
+
+// density-weighted horizontal statistics (App. B): out[Ez*Nq][20], see favre_profiles
+void odg_profiles(void* h, const double* Q, double* out) { favre_profiles(*(Ctx*)h, Q, out); }
 
 int odg_num_threads() {
   int n = 1;

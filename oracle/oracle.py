@@ -39,6 +39,7 @@ class _Params(C.Structure):
         ("richardson", C.c_int32), ("p_0", C.c_double),
         ("sponge_alpha", C.c_double), ("sponge_zs", C.c_double), ("sponge_gamma", C.c_int32), ("u_relax", C.c_double * 3),
         ("filter_order", C.c_int32), ("filter_alpha", C.c_double), ("riemann", C.c_int32), ("metric_form", C.c_int32),
+        ("drag_cd", C.c_double), ("lhf_bottom", C.c_double), ("evap_bottom", C.c_double),
     ]
 
 
@@ -83,6 +84,7 @@ def lib():
             "odg_euler": [C.c_void_p, _dp, C.c_double, C.c_int],
             "odg_lsrk54_stage": [C.c_void_p, _dp, _dp, C.c_double, C.c_int],
             "odg_diagnostics": [C.c_void_p, _dp, _dp],
+            "odg_profiles": [C.c_void_p, _dp, _dp],
         }.items():
             getattr(L, name).argtypes = args
             getattr(L, name).restype = None
@@ -166,6 +168,8 @@ class Oracle:
         p.u_relax[:] = [float(v) for v in cfg.get("u_relax", (0.0, 0.0, 0.0))]
         p.filter_order = int(cfg.get("filter_order", 0)); p.filter_alpha = float(cfg.get("filter_alpha", 36.0436533891172))
         p.riemann = int(cfg.get("riemann", 0)); p.metric_form = int(cfg.get("metric_form", 0))
+        p.drag_cd = float(cfg.get("drag_cd", 0.0)); p.lhf_bottom = float(cfg.get("lhf_bottom", 0.0))
+        p.evap_bottom = float(cfg.get("evap_bottom", 0.0))
         self._h = L.odg_create(C.byref(p))
         if not self._h:
             raise ValueError("odg_create rejected the parameters")
@@ -293,3 +297,11 @@ class Oracle:
         Q = self._q(Q); out = np.zeros(8)
         lib().odg_diagnostics(self._h, _ptr(Q), _ptr(out))
         return dict(zip(("mass", "energy", "water", "kinetic", "max_wavespeed", "min_node_dx", "volume", "n_nonfinite"), out))
+
+    PROFILE_COLUMNS = ("z", "rho") + tuple(f"{p}{v}" for p in ("", "w'", "var_") for v in ("u", "v", "w", "h_tot", "q_t", "theta_v"))
+
+    def profiles(self, Q):
+        """Density-weighted horizontal statistics (App. B): array [Ez*Nq][20], columns PROFILE_COLUMNS."""
+        Q = self._q(Q); out = np.zeros((self.ne[2] * self.Nq, 20))
+        lib().odg_profiles(self._h, _ptr(Q), _ptr(out))
+        return out
