@@ -149,6 +149,10 @@ __device__ __forceinline__ void cm10_cp_arrive(uint64_t* bar) {   // arrive on b
 __device__ __forceinline__ void cm10_bar_compute(int nthreads) {   // barrier among the compute warps only (id 1)
   asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
 }
+// "buffers free" hand-over (id 2): the compute warps only ARRIVE (they never wait for the producer's instruction stream,
+// only for its data), the producer warp waits until every compute thread has arrived
+__device__ __forceinline__ void cm10_bar_release(int nthreads) { asm volatile("bar.arrive 2, %0;" ::"r"(nthreads) : "memory"); }
+__device__ __forceinline__ void cm10_bar_acquire(int nthreads) { asm volatile("bar.sync 2, %0;" ::"r"(nthreads) : "memory"); }
 
 // lifted numerical-flux part of one face node from the two states (cm7_tend_face with the operands in registers):
 //   rf[v] = -(1/2) sJ n.F^+[v] - (1/2) sJ lambda (Y^-[v] - Y^+[v])          interior / periodic (eq. 27 with R1, R2, R6)
@@ -264,7 +268,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS + 32, CmCfg10<Nq, M
     };
     if (R::NTB == 2) gather(0);
     for (int j = 0; j < S; ++j) {
-      __syncthreads();                                 // the compute warps are done with every buffer of element j-1
+      cm10_bar_acquire(THREADS + 32);                  // the compute warps are done with every buffer of element j-1
       if (lane == 0) {
         cm10_fence_proxy_async();                      // generic-proxy accesses of the buffers before the async-proxy writes
         if (j + 1 < S) issue_tile(j + 1, (j + 1) & 1);
@@ -308,27 +312,25 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS + 32, CmCfg10<Nq, M
     const int sh = C::ODD ? (e & 1) : 0;
     const int wm = row.pos.wallmask | ((it == 0 && row.wallL) ? 1 : 0) | ((it == S - 1 && row.wallR) ? 2 : 0);
     const bool more = it + 1 < S;
-    __syncthreads();                                   // releases the buffers of the previous iteration to the producer
+    // releases the buffers of the previous iteration to the producer WITHOUT waiting: a warp that has finished phase 3
+    // starts phase 1 of the next element at once.  What phase 1 writes is either private to the thread's own node (F^2,
+    // c) or lies in the other tile buffer; the xi- carry is written behind the first compute barrier for this reason.
+    cm10_bar_release(THREADS + 32);
     cm7_mbar_wait(mbar + b, (it >> 1) & 1);
 
     double* Qs = Qb + b * NV * SLOT + sh; double* Fs = Gb + b * 2 * NV * SLOT; double* cs = ct;   // G is element-major: no shift
     // ---- phase 1: primitives and contravariant fluxes of the own node (F^1, F^3 overwrite G in place)
     double buoy = 0.0;
-    double Y[6];
+    double Y[6], gc[5];
     if (node) {
       double g[12]; CmPrim P;
 #pragma unroll
       for (int v = 0; v < NV; ++v) Y[v] = Qs[v * SLOT + n];
-      if (SGS)
+      if (SGS) {
 #pragma unroll
         for (int k = 0; k < NG; ++k) g[k] = Fs[k * SLOT + n];
-      if (i_ == N && more) {                           // the i = N plane is the xi- trace of the next element
-        double* xl = X + (b ^ 1) * XS + (j_ + Nq * k_);
 #pragma unroll
-        for (int v = 0; v < NV; ++v) xl[v * NF] = Y[v];
-        if (SGS)
-#pragma unroll
-          for (int k = 0; k < NGD; ++k) xl[(NV + k) * NF] = g[cm7_gidx(0, k)];
+        for (int k = 0; k < NGD; ++k) gc[k] = g[cm7_gidx(0, k)];
       }
       cm_eos<MOIST>(p, Y, st, P);
       buoy = P.drho * p.th.grav;
@@ -341,6 +343,14 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS + 32, CmCfg10<Nq, M
       for (int v = 0; v < NV; ++v) { Fs[v * SLOT + n] = Fa[v]; Fs[(NV + v) * SLOT + n] = Fc[v]; F2[v * C::SLOT2 + n2] = Fb[v]; }
     }
     cm10_bar_compute(THREADS);
+    if (node && i_ == N && more) {                     // the i = N plane is the xi- trace of the next element (every warp
+      double* xl = X + (b ^ 1) * XS + (j_ + Nq * k_);  // has left phase 3 of the previous element, which read this block)
+#pragma unroll
+      for (int v = 0; v < NV; ++v) xl[v * NF] = Y[v];
+      if (SGS)
+#pragma unroll
+        for (int k = 0; k < NGD; ++k) xl[(NV + k) * NF] = gc[k];
+    }
 
     // ---- phase 2: line tasks, then face tasks
     for (int lt = t; lt < 3 * NFP; lt += THREADS) {
@@ -401,15 +411,17 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS + 32, CmCfg10<Nq, M
       }
       const int c3[3] = {i_, j_, k_};
       const int m3[3] = {j_ + Nq * k_, i_ + Nq * k_, i_ + Nq * j_};
+      double lf[3][6];                                 // rf of the up to three faces through the node: independent
+#pragma unroll                                         // (predicated) loads, all in flight together
+      for (int d = 0; d < 3; ++d) {
+        const bool on = c3[d] == 0 || c3[d] == N, hi = c3[d] == N;
+        const double* tr = (d == 0) ? (hi ? X + 2 * XS : X + b * XS) : T + (it % R::NTB) * 4 * TS + (2 * d - 2 + (hi ? 1 : 0)) * TS;
+        tr += m3[d];
 #pragma unroll
-      for (int d = 0; d < 3; ++d)
-        if (c3[d] == 0 || c3[d] == N) {
-          const bool hi = c3[d] == N;
-          const double* tr = (d == 0) ? (hi ? X + 2 * XS : X + b * XS) : T + (it % R::NTB) * 4 * TS + (2 * d - 2 + (hi ? 1 : 0)) * TS;
-          tr += m3[d];
+        for (int v = 0; v < NV; ++v) lf[d][v] = on ? tr[v * NF] : 0.0;
+      }
 #pragma unroll
-          for (int v = 0; v < NV; ++v) lift[v] += tr[v * NF];
-        }
+      for (int v = 0; v < NV; ++v) lift[v] = (lf[0][v] + lf[1][v]) + lf[2][v];
       const size_t idx = (size_t)e * NP + n;
       double* o1 = (MODE == 0) ? p.dQ + idx : p.dQ + (size_t)e * (NV * SLOT) + n;
       const long long s1 = (MODE == 0) ? p.stride : (long long)SLOT;
