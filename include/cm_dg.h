@@ -76,6 +76,12 @@ typedef struct {
                                stored-metric kernels                                                          */
   int32_t metric_form;      /* 0 cross-product metric terms (extruded / 2.5-D warps) | 1 curl-invariant form
                                (fully 3-D warps; geom == 2)                                                   */
+  /* ---- surface fluxes through the z-low wall (App. A1; need bc[2] == 1); all-zero = free slip, no flux ---- */
+  double drag_cd;           /* C_d of the aerodynamic drag law, eq. (A2): n.(rho tau) = -rho C_d |u_p,int| u_p,int
+                               with u_p,int the wall-parallel velocity at the first layer of interior nodes          */
+  double lhf_bottom;        /* W m^-2 latent heat flux, added to shf_bottom in the wall energy flux   */
+  double evap_bottom;       /* kg m^-2 s^-1 evaporation E = n.(rho d_qv)|sfc into the domain: enters the
+                               rho*q_tot and rho equations (nvar == 6); the caller derives it from LHF                */
 } cm_dg_params;
 
 /* Optional scheduling knobs (HOST, copied by cm_dg_setup_tuned).  They never change what is computed (the parity tests
@@ -157,6 +163,17 @@ int cm_dg_filter(cm_dg_ctx* ctx, double* Q_dev);
 
 /* a6: conservation integrals etc. of Q_dev into *out_host; synchronises the stream. */
 int cm_dg_diagnostics(cm_dg_ctx* ctx, const double* Q_dev, cm_dg_diag* out_host);
+
+/* Density-weighted horizontal statistics of App. B (eq. B1-B4) on the nodal mesh.  Levels are the nodal
+ * zeta-planes of every element layer, l = ez * Nq + k (nlev = Ez * Nq; the two planes of an element interface are separate
+ * levels); <a>_l = sum W a / sum W over the plane with W = w_i w_j |Ja^3| (area element of the zeta = const surface).
+ * out_host is HOST [nlev][CM_DG_NPROF], columns: <z>, <rho>, then for phi = u, v, w, h_tot, q_tot, theta_v the Favre mean
+ * phibar = <rho phi>/<rho> (B1), the vertical eddy flux <rho w' phi'>/<rho> (B2) and the variance <rho phi'^2>/<rho> (B4),
+ * phi' = phi - phibar (B3): 2 + 3 * 6 columns.  Two sweeps over Q_dev (means, then fluctuations), summed in a fixed order
+ * (bitwise repeatable).  Uses the LSRK residual buffer as scratch; synchronises the stream.
+ * CM_DG_EINVAL if nlev_capacity < Ez * Nq. */
+#define CM_DG_NPROF 20
+int cm_dg_profiles(cm_dg_ctx* ctx, const double* Q_dev, double* out_host, int32_t nlev_capacity);
 
 /* End-to-end variants on HOST buffers in the same [nvar][field_stride] layout (pinned memory recommended):
  * host->device copy, the device call above, device->host copy, stream synchronise. */

@@ -7,5 +7,5 @@ There is no CPU fallback: importing ``binding`` fails loudly if the library has 
 """
 from .binding import (CmDg, CmDgError, cm_dg_coords, cm_dg_destroy, cm_dg_diagnostics, cm_dg_gradient,  # noqa: F401
                       cm_dg_last_error, cm_dg_layout, cm_dg_lsrk_step, cm_dg_lsrk_step_host, cm_dg_lsrk_step_table, cm_dg_filter,
-                      cm_dg_metrics,
+                      cm_dg_metrics, cm_dg_profiles,
                       cm_dg_profile_begin, cm_dg_profile_end, cm_dg_rhs, cm_dg_rhs_host, cm_dg_setup, library_path)  # noqa: F401

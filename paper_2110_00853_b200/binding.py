@@ -26,6 +26,7 @@ class _Params(C.Structure):
         ("richardson", C.c_int32), ("p_0", C.c_double),
         ("sponge_alpha", C.c_double), ("sponge_zs", C.c_double), ("sponge_gamma", C.c_int32), ("u_relax", C.c_double * 3),
         ("filter_order", C.c_int32), ("filter_alpha", C.c_double), ("riemann", C.c_int32), ("metric_form", C.c_int32),
+        ("drag_cd", C.c_double), ("lhf_bottom", C.c_double), ("evap_bottom", C.c_double),
     ]
 
 
@@ -46,7 +47,7 @@ class _KStats(C.Structure):
 
 
 EXPORTS = ("cm_dg_setup", "cm_dg_setup_tuned", "cm_dg_layout", "cm_dg_coords", "cm_dg_metrics", "cm_dg_gradient", "cm_dg_rhs",
-           "cm_dg_lsrk_step", "cm_dg_lsrk_step_table", "cm_dg_filter", "cm_dg_diagnostics", "cm_dg_rhs_host", "cm_dg_lsrk_step_host",
+           "cm_dg_lsrk_step", "cm_dg_lsrk_step_table", "cm_dg_filter", "cm_dg_diagnostics", "cm_dg_profiles", "cm_dg_rhs_host", "cm_dg_lsrk_step_host",
            "cm_dg_profile_begin", "cm_dg_profile_end", "cm_dg_destroy", "cm_dg_last_error")
 
 _lib = None
@@ -76,6 +77,7 @@ def _load():
     L.cm_dg_lsrk_step_table.argtypes = [vp, vp, dbl, dbl, i32, i32, vp, vp, vp]
     L.cm_dg_filter.argtypes = [vp, vp]
     L.cm_dg_diagnostics.argtypes = [vp, vp, C.POINTER(_Diag)]
+    L.cm_dg_profiles.argtypes = [vp, vp, vp, i32]
     L.cm_dg_rhs_host.argtypes = [vp, vp, vp, dbl]
     L.cm_dg_lsrk_step_host.argtypes = [vp, vp, dbl, dbl, i32]
     L.cm_dg_profile_begin.argtypes = [vp]
@@ -147,7 +149,7 @@ def cm_dg_setup(cfg, stream=None, tuning=None):
     p.sgs = int(cfg.get("sgs", 0))
     for k in ("richardson", "sponge_gamma", "filter_order", "riemann", "metric_form"):
         setattr(p, k, int(cfg.get(k, 0)))
-    for k in ("p_0", "sponge_alpha", "sponge_zs", "filter_alpha"):
+    for k in ("p_0", "sponge_alpha", "sponge_zs", "filter_alpha", "drag_cd", "lhf_bottom", "evap_bottom"):
         setattr(p, k, float(cfg.get(k, 0.0)))
     p.u_relax[:] = [float(v) for v in cfg.get("u_relax", (0.0, 0.0, 0.0))]
     p.use_ref = int(cfg.get("use_ref", 0))
@@ -212,6 +214,16 @@ def cm_dg_diagnostics(ctx, Q_dev):
     d = _Diag()
     _check(_load().cm_dg_diagnostics(ctx, _dptr(Q_dev), C.byref(d)), "cm_dg_diagnostics")
     return {k: getattr(d, k) for k, _ in _Diag._fields_}
+
+
+NPROF = 20   # CM_DG_NPROF
+
+
+def cm_dg_profiles(ctx, Q_dev, out_host):
+    """out_host: numpy float64 [nlev][NPROF] (nlev >= Ez * Nq)."""
+    assert out_host.ndim == 2 and out_host.shape[1] == NPROF
+    _check(_load().cm_dg_profiles(ctx, _dptr(Q_dev), _hptr(out_host), int(out_host.shape[0])), "cm_dg_profiles")
+    return out_host
 
 
 def cm_dg_rhs_host(ctx, Q_host, dQ_host, t=0.0):
@@ -313,6 +325,11 @@ class CmDg:
 
     def diagnostics(self, Q):
         return cm_dg_diagnostics(self.ctx, Q)
+
+    def profiles(self, Q):
+        """Density-weighted horizontal statistics (App. B): numpy [Ez * Nq][NPROF]."""
+        out = np.zeros((int(self.cfg["ne"][2]) * (int(self.cfg["N"]) + 1), NPROF))
+        return cm_dg_profiles(self.ctx, Q, out)
 
     def rhs_host(self, Q_host, dQ_host, t=0.0):
         cm_dg_rhs_host(self.ctx, Q_host, dQ_host, t)

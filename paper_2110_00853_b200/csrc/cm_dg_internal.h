@@ -55,7 +55,9 @@ struct CmKP {
   double d2[3];          // flat: squared mixing lengths Delta_m^2 = (h_m / N)^2 of the Vreman model (eq. 39c)
   double urelax[3];      // Rayleigh sponge: relaxation velocity (eq. A4); tau_s comes with the z table / geometry
   double inv_Pr;
-  double shf;            // prescribed upward energy flux at the bottom wall
+  double shf;            // prescribed upward energy flux at the bottom wall: SHF + LHF
+  double evap;           // prescribed evaporation E through the bottom wall [kg m^-2 s^-1]
+  double drag_cd;        // drag coefficient C_d of eq. (A2) on the bottom wall, 0 = free slip
   double inv_w0;         // 1 / w_0 = N (N+1) / 2
   double rka, rkb, dt;   // LSRK stage coefficients
   double D[CM_MAXNQ][CM_MAXNQ];  // D[i][m] = L_m'(xi_i)

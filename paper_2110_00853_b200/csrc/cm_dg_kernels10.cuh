@@ -160,7 +160,7 @@ __device__ __forceinline__ void cm10_bar_acquire(int nthreads) { asm volatile("b
 template <int Nq, bool MOIST, bool SGS>
 __device__ __forceinline__ void cm10_face_flux(const CmKP& p, const double (&Ym)[6], double cm_, const double (&Yp)[6],
                                                const double (&gp)[5], const double* __restrict__ zt, bool wall, int f, int d,
-                                               int s, int kline, double (&rf)[6]) {
+                                               int s, int kline, const double* __restrict__ qint, double (&rf)[6]) {
   using C = CmCfg7<Nq, MOIST>;
   constexpr int NV = C::NV;
   const double sgn = s ? 1.0 : -1.0;
@@ -199,7 +199,10 @@ __device__ __forceinline__ void cm10_face_flux(const CmKP& p, const double (&Ym)
 #pragma unroll
     for (int v = 0; v < NV; ++v) rf[v] = 0.0;
     rf[1] = (d == 0) ? mom : 0.0; rf[2] = (d == 1) ? mom : 0.0; rf[3] = (d == 2) ? mom : 0.0;
-    if (f == 4) rf[4] = sJ * p.shf;                                        // prescribed upward energy flux
+    if (f == 4) {                                                          // prescribed surface fluxes, drag law (App. A1);
+      const double Aw[3] = {0.0, 0.0, -sJ};                                // qint: the node above the wall node in the own tile
+      cm_surface_flux<MOIST>(p, Aw, sJ, Ym[0], qint, CmCfg7<Nq, MOIST>::SLOT, rf);
+    }
   }
 }
 
@@ -392,7 +395,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS + 32, CmCfg10<Nq, M
             for (int k = 0; k < NGD; ++k) gp[k] = out[(NV + k) * NF];
         }
       }
-      cm10_face_flux<Nq, MOIST, SGS>(p, Ym, cm_, Yp, gp, zt, wall, f, d, s, kline, rf);
+      cm10_face_flux<Nq, MOIST, SGS>(p, Ym, cm_, Yp, gp, zt, wall, f, d, s, kline, Qs + nm + NF, rf);
 #pragma unroll
       for (int v = 0; v < NV; ++v) out[v * NF] = rf[v];
     }

@@ -335,7 +335,7 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_ten
 #pragma unroll
           for (int v = 0; v < NV; ++v) r[v] = Ftm[v] - Fs[v];
         }
-        if (f == 4) r[4] += sJ * p.shf;
+        if (f == 4) cm_surface_flux<MOIST>(p, A, sJ, Ym[0], qm + NF, NP, r);   // the node above nm: first interior layer
       }
       double* fb = fbuf + ((size_t)el * 6 * NF + ft) * NV;
 #pragma unroll

@@ -305,7 +305,10 @@ __device__ __forceinline__ void cm7_tend_face(const CmKP& p, const double* __res
 #pragma unroll
     for (int v = 0; v < NV; ++v) rf[v] = 0.0;
     rf[1] = (d == 0) ? mom : 0.0; rf[2] = (d == 1) ? mom : 0.0; rf[3] = (d == 2) ? mom : 0.0;
-    if (f == 4) rf[4] = sJ * p.shf;                                        // prescribed upward energy flux
+    if (f == 4) {                                                          // prescribed surface fluxes, drag law (App. A1)
+      const double Aw[3] = {0.0, 0.0, -sJ};
+      cm_surface_flux<MOIST>(p, Aw, sJ, Ym[0], Qs + nm + NF, SLOT, rf);
+    }
   }
 #pragma unroll
   for (int v = 0; v < NV; ++v) tr[v * NF] = rf[v];

@@ -368,6 +368,130 @@ __global__ void filter_kernel(const __grid_constant__ FilterArgs a) {
   }
 }
 
+// a6, second stage: the per-element partial sums are reduced on the device in a fixed order (thread t takes elements
+// t, t + T, ...; then a fixed tree), so only 7 doubles travel to the host
+__global__ void diag_reduce_kernel(long long Ne, const double* __restrict__ part, double* __restrict__ out) {
+  __shared__ double sh[7][256];
+  double r[7] = {0, 0, 0, 0, 0, 0, 0};
+  for (long long e = threadIdx.x; e < Ne; e += blockDim.x)
+    for (int m = 0; m < 7; ++m) { const double v = part[7 * e + m]; r[m] = (m == 5) ? fmax(r[m], v) : r[m] + v; }
+  for (int m = 0; m < 7; ++m) sh[m][threadIdx.x] = r[m];
+  __syncthreads();
+  for (int s = blockDim.x / 2; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s)
+      for (int m = 0; m < 7; ++m) sh[m][threadIdx.x] = (m == 5) ? fmax(sh[m][threadIdx.x], sh[m][threadIdx.x + s]) : sh[m][threadIdx.x] + sh[m][threadIdx.x + s];
+    __syncthreads();
+  }
+  if (threadIdx.x < 7) out[threadIdx.x] = sh[threadIdx.x][0];
+}
+
+// App. B statistics (eq. B1-B4).  pass 0: per element and nodal zeta-plane the sums of W [1, z, rho, rho phi_m];
+// pass 1: of W rho [w' phi'_m, phi'_m^2] with the level means of pass 0.  W = w_i w_j |Ja^3|.
+struct ProfArgs {
+  int Nq, Np, nvar, general, pass;
+  long long Ne, stride;
+  const double* Q; const double* geo; const int* erow; const double* ztab;
+  const double* lev;                 // pass 1: [nlev][CM_DG_NPROF] level means
+  double A3flat, grav; double w[CM_MAXNQ];
+  CmThermo th;
+};
+constexpr int PROF_NS0 = 9, PROF_NS1 = 12;
+
+__device__ inline void prof_vars(const ProfArgs& a, const double* Y, double Phi, double* phi) {
+  const CmThermo& th = a.th;
+  const double ir = 1.0 / Y[0];
+  const double u = Y[1] * ir, v = Y[2] * ir, w = Y[3] * ir;
+  const double rq = (a.nvar == 6) ? Y[5] : 0.0, q = rq * ir;
+  const double K = 0.5 * (Y[1] * u + Y[2] * v + Y[3] * w);
+  const double kappa = (th.R_d + th.a * q) / (th.c_vd + th.b * q);
+  const double E = Y[4] - K - Y[0] * Phi - rq * th.I_v0;
+  const double pr = kappa * E + th.T_0 * (th.R_d * Y[0] + th.a * rq);
+  phi[0] = u; phi[1] = v; phi[2] = w; phi[3] = (Y[4] + pr) * ir; phi[4] = q;
+  phi[5] = pr * ir * th.iRd * pow(th.p_0 / pr, th.kap_pd);          // theta_v without condensate (R25)
+}
+
+__global__ void prof_kernel(const __grid_constant__ ProfArgs a, double* __restrict__ part) {
+  extern __shared__ double sh[];                                     // [NF][ns]
+  const long long e = blockIdx.x;
+  const int Nq = a.Nq, NF = Nq * Nq, ns = a.pass ? PROF_NS1 : PROF_NS0;
+  const int ez_row = a.erow[e];                                      // ez * Nq
+  for (int k = 0; k < Nq; ++k) {
+    for (int m = threadIdx.x; m < NF; m += blockDim.x) {
+      const int n = m + NF * k, i = m % Nq, j = m / Nq;
+      const long long idx = e * a.Np + n;
+      double Y[6] = {0, 0, 0, 0, 0, 0};
+      for (int v = 0; v < a.nvar; ++v) Y[v] = a.Q[v * a.stride + idx];
+      double z, A3;
+      if (a.general) {
+        z = a.geo[10 * a.stride + idx];
+        const double a0 = a.geo[6 * a.stride + idx], a1 = a.geo[7 * a.stride + idx], a2 = a.geo[8 * a.stride + idx];
+        A3 = sqrt(a0 * a0 + a1 * a1 + a2 * a2);
+      } else {
+        z = 0.0;                                                      // flat: the level height is known in closed form
+        A3 = a.A3flat;
+      }
+      const double Phi = a.general ? a.grav * z : a.ztab[(long long)(ez_row + k) * CM_ZTAB_W];
+      const double W = a.w[i] * a.w[j] * A3;
+      double phi[6]; prof_vars(a, Y, Phi, phi);
+      double* o = sh + m * ns;
+      if (a.pass == 0) {
+        o[0] = W; o[1] = W * z; o[2] = W * Y[0];
+        for (int q = 0; q < 6; ++q) o[3 + q] = W * Y[0] * phi[q];
+      } else {
+        const double* L = a.lev + (long long)(ez_row + k) * CM_DG_NPROF;
+        const double wp = phi[2] - L[2 + 2];
+        for (int q = 0; q < 6; ++q) {
+          const double fp = phi[q] - L[2 + q];
+          o[q] = W * Y[0] * wp * fp; o[6 + q] = W * Y[0] * fp * fp;
+        }
+      }
+    }
+    __syncthreads();
+    if ((int)threadIdx.x < ns) {
+      double s = 0.0;
+      for (int m = 0; m < NF; ++m) s += sh[m * ns + threadIdx.x];
+      part[(e * Nq + k) * ns + threadIdx.x] = s;
+    }
+    __syncthreads();
+  }
+}
+
+// one CTA per level: sums the partials of the Ex*Ey elements of the layer in a fixed order, then normalises
+struct ProfRedArgs { int Nq, pass, Ex, Ey, Ez, L, PY, NXC; double flat_dz0, flat_lo, flat_h; int flat_z; double xi[CM_MAXNQ]; };
+
+__global__ void prof_reduce_kernel(const __grid_constant__ ProfRedArgs a, const double* __restrict__ part, double* __restrict__ lev,
+                                   double* __restrict__ sumW) {
+  __shared__ double sh[PROF_NS1][256];
+  const int l = blockIdx.x, ez = l / a.Nq, k = l - ez * a.Nq, ns = a.pass ? PROF_NS1 : PROF_NS0;
+  double r[PROF_NS1];
+  for (int q = 0; q < PROF_NS1; ++q) r[q] = 0.0;
+  for (int h = threadIdx.x; h < a.Ex * a.Ey; h += blockDim.x) {
+    const int ex = h % a.Ex, ey = h / a.Ex;
+    const long long e = ((((long long)(ey / a.PY) * a.NXC + ex / a.L) * a.Ez + ez) * a.PY + ey % a.PY) * a.L + ex % a.L;
+    const double* p = part + (e * a.Nq + k) * ns;
+    for (int q = 0; q < ns; ++q) r[q] += p[q];
+  }
+  for (int q = 0; q < ns; ++q) sh[q][threadIdx.x] = r[q];
+  __syncthreads();
+  for (int s = blockDim.x / 2; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s) for (int q = 0; q < ns; ++q) sh[q][threadIdx.x] += sh[q][threadIdx.x + s];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    double* o = lev + (long long)l * CM_DG_NPROF;
+    if (a.pass == 0) {
+      const double sw = sh[0][0];
+      sumW[l] = sw;
+      o[0] = a.flat_z ? a.flat_lo + (ez + 0.5 * (a.xi[k] + 1.0)) * a.flat_h : sh[1][0] / sw;
+      o[1] = sh[2][0] / sw;
+      for (int q = 0; q < 6; ++q) o[2 + q] = (sh[3 + q][0] / sw) / o[1];        // (B1)
+    } else {
+      const double sw = sumW[l];
+      for (int q = 0; q < 12; ++q) o[8 + q] = (sh[q][0] / sw) / o[1];           // (B2), (B4)
+    }
+  }
+}
+
 }  // namespace
 
 struct cm_dg_ctx {
@@ -386,6 +510,8 @@ struct cm_dg_ctx {
   int *d_nbr = nullptr, *d_erow = nullptr, *d_lex = nullptr;
   double *d_ztab = nullptr, *d_geo = nullptr, *d_ref = nullptr, *d_G = nullptr, *d_res = nullptr, *d_Q2 = nullptr, *d_Q3 = nullptr;
   double *d_zsfc = nullptr, *d_xyz_user = nullptr, *d_part = nullptr, *d_stage = nullptr;
+  double *d_lev = nullptr;         // [Ez*Nq][CM_DG_NPROF] level statistics + [Ez*Nq] sum of weights + 7 reduced diagnostics
+  int tileL = 1, tilePY = 1;       // the tiled element order (x-chunk, y-patch)
   CmKP kp;
   cm_launch_fn launch_grad = nullptr, launch_tend = nullptr;
   int ahead_t = -1, ahead_g = -1;   // L2 prefetch distance of the tendency / gradient kernel (-1 = one wave)
@@ -402,7 +528,7 @@ void free_ctx(cm_dg_ctx* c) {
   if (!c) return;
   cudaFree(c->d_nbr); cudaFree(c->d_erow); cudaFree(c->d_lex); cudaFree(c->d_ztab); cudaFree(c->d_geo);
   cudaFree(c->d_ref); cudaFree(c->d_G); cudaFree(c->d_res); cudaFree(c->d_Q2); cudaFree(c->d_Q3); cudaFree(c->d_zsfc);
-  cudaFree(c->d_xyz_user); cudaFree(c->d_part); cudaFree(c->d_stage);
+  cudaFree(c->d_xyz_user); cudaFree(c->d_part); cudaFree(c->d_stage); cudaFree(c->d_lev);
   for (auto e : c->ev) cudaEventDestroy(e);
   delete c;
 }
@@ -515,6 +641,9 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   if (p->sponge_alpha < 0.0 || p->sponge_gamma < 0) return fail(CM_DG_EINVAL, "cm_dg_setup: sponge_alpha and sponge_gamma must be >= 0");
   if (p->sponge_alpha > 0.0 && !(p->sponge_zs < p->hi[2])) return fail(CM_DG_EINVAL, "cm_dg_setup: the sponge must start below hi[2]");
   if (!(p->c_vd > 0.0) || !(p->R_d > 0.0)) return fail(CM_DG_EINVAL, "cm_dg_setup: R_d and c_vd must be positive");
+  if (p->drag_cd < 0.0) return fail(CM_DG_EINVAL, "cm_dg_setup: drag_cd must be >= 0");
+  if ((p->drag_cd != 0.0 || p->lhf_bottom != 0.0 || p->evap_bottom != 0.0) && p->bc[2] != 1)
+    return fail(CM_DG_EINVAL, "cm_dg_setup: surface fluxes (drag_cd, lhf_bottom, evap_bottom) need a wall in z (bc[2] == 1)");
   const int64_t Ne = (int64_t)p->ne[0] * p->ne[1] * p->ne[2];
   const int Nq = p->N + 1, Np = Nq * Nq * Nq;
   if (Ne * Np >= (int64_t)1 << 31) return fail(CM_DG_EINVAL, "cm_dg_setup: more than 2^31 nodes");
@@ -642,6 +771,7 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   std::memset(&kp, 0, sizeof(kp));
   kp.ginvL = 1.0f / (float)L; kp.ginvNXC = 1.0f / (float)(p->ne[0] / L);
   kp.gL = L; kp.gPY = PY; kp.gNXC = p->ne[0] / L; kp.gNYP = p->ne[1] / PY; kp.gEz = p->ne[2];
+  c->tileL = L; c->tilePY = PY;
   for (int d = 0; d < 3; ++d) kp.gbc[d] = p->bc[d];
   kp.ahead = -1;   // L2 prefetch distance of the cm7 kernels: -1 = one wave of resident CTAs (set by the launcher)
   c->ahead_t = tn.ahead_t; c->ahead_g = tn.ahead_g;
@@ -670,7 +800,8 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
     kp.cs2delta2 = (p->C_s * delta) * (p->C_s * delta);
   }
   kp.inv_Pr = p->sgs ? 1.0 / p->Pr_t : 0.0;
-  kp.shf = p->shf_bottom;
+  kp.shf = p->shf_bottom + p->lhf_bottom;   // n_in . rho (J + D) = SHF + LHF
+  kp.evap = p->evap_bottom; kp.drag_cd = p->drag_cd;
   kp.inv_w0 = 1.0 / c->w[0];
   for (int i = 0; i < CM_MAXNQ; ++i) for (int j = 0; j < CM_MAXNQ; ++j) kp.D[i][j] = c->D[i][j];
   kp.nbr = c->d_nbr; kp.erow = c->d_erow;
@@ -746,6 +877,7 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   c->em_bytes_per_field = std::max(fbytes, (size_t)Ne * slot * sizeof(double));
   if (p->sgs) CM_CUDA_B(cudaMalloc(&c->d_G, (size_t)c->ngrad * c->em_bytes_per_field));
   CM_CUDA_B(cudaMalloc(&c->d_part, (size_t)Ne * 7 * sizeof(double)));
+  CM_CUDA_B(cudaMalloc(&c->d_lev, ((size_t)p->ne[2] * Nq * (CM_DG_NPROF + 1) + 8) * sizeof(double)));
   // LSRK residual and the two further state buffers of the stage ring (cm_dg_lsrk_step never allocates or synchronises)
   {
     const size_t sb = (size_t)c->nvar * fbytes;
@@ -873,14 +1005,48 @@ int cm_dg_diagnostics(cm_dg_ctx* ctx, const double* Q_dev, cm_dg_diag* out) {
     diag_kernel<<<(unsigned)ctx->Ne, thr, 7 * thr * sizeof(double), ctx->st>>>(a, ctx->d_part);
   }
   CM_CUDA(cudaGetLastError());
-  std::vector<double> part((size_t)ctx->Ne * 7);
-  CM_CUDA(cudaMemcpyAsync(part.data(), ctx->d_part, part.size() * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
-  CM_CUDA(cudaStreamSynchronize(ctx->st));
+  double* d_red = ctx->d_lev + (size_t)ctx->prm.ne[2] * ctx->Nq * (CM_DG_NPROF + 1);
+  {
+    Timed tm(ctx, 2);
+    diag_reduce_kernel<<<1, 256, 0, ctx->st>>>(ctx->Ne, ctx->d_part, d_red);
+  }
+  CM_CUDA(cudaGetLastError());
   double s[7] = {0, 0, 0, 0, 0, 0, 0};
-  for (int64_t e = 0; e < ctx->Ne; ++e)
-    for (int m = 0; m < 7; ++m) s[m] = (m == 5) ? std::max(s[m], part[7 * e + m]) : s[m] + part[7 * e + m];
+  CM_CUDA(cudaMemcpyAsync(s, d_red, sizeof(s), cudaMemcpyDeviceToHost, ctx->st));
+  CM_CUDA(cudaStreamSynchronize(ctx->st));
   out->mass = s[0]; out->energy = s[1]; out->water = s[2]; out->kinetic = s[3] / s[4]; out->volume = s[4];
   out->max_wavespeed = s[5]; out->n_nonfinite = (int64_t)s[6]; out->min_node_dx = ctx->min_node_dx;
+  return CM_DG_OK;
+}
+
+int cm_dg_profiles(cm_dg_ctx* ctx, const double* Q_dev, double* out, int32_t nlev_capacity) {
+  if (!ctx || !Q_dev || !out) return fail(CM_DG_EINVAL, "cm_dg_profiles: NULL argument");
+  { int rc_ = enter(ctx, "cm_dg_profiles"); if (rc_) return rc_; }
+  const int nlev = ctx->prm.ne[2] * ctx->Nq;
+  if (nlev_capacity < nlev) return fail(CM_DG_EINVAL, "cm_dg_profiles: out_host holds fewer than Ez * Nq levels");
+  ProfArgs a;
+  a.Nq = ctx->Nq; a.Np = ctx->Np; a.nvar = ctx->nvar; a.general = ctx->general;
+  a.Ne = ctx->Ne; a.stride = ctx->stride; a.Q = Q_dev; a.geo = ctx->d_geo; a.erow = ctx->d_erow; a.ztab = ctx->d_ztab;
+  a.lev = ctx->d_lev; a.A3flat = ctx->kp.cA[2]; a.grav = ctx->prm.grav;
+  for (int i = 0; i < CM_MAXNQ; ++i) a.w[i] = ctx->w[i];
+  a.th = ctx->kp.th;
+  ProfRedArgs r;
+  r.Nq = ctx->Nq; r.Ex = ctx->prm.ne[0]; r.Ey = ctx->prm.ne[1]; r.Ez = ctx->prm.ne[2];
+  r.L = ctx->tileL; r.PY = ctx->tilePY; r.NXC = r.Ex / r.L;
+  r.flat_z = ctx->general ? 0 : 1; r.flat_lo = ctx->prm.lo[2]; r.flat_h = ctx->h[2]; r.flat_dz0 = 0.0;
+  for (int i = 0; i < CM_MAXNQ; ++i) r.xi[i] = ctx->xi[i];
+  double* part = ctx->d_res;                               // scratch: Ne * Nq * 12 <= Ne * Np * nvar doubles
+  double* sumW = ctx->d_lev + (size_t)nlev * CM_DG_NPROF;
+  const int NF = ctx->Nq * ctx->Nq;
+  for (int pass = 0; pass < 2; ++pass) {
+    a.pass = r.pass = pass;
+    Timed tm(ctx, 2);
+    prof_kernel<<<(unsigned)ctx->Ne, 64, (size_t)NF * PROF_NS1 * sizeof(double), ctx->st>>>(a, part);
+    prof_reduce_kernel<<<(unsigned)nlev, 256, 0, ctx->st>>>(r, part, ctx->d_lev, sumW);
+  }
+  CM_CUDA(cudaGetLastError());
+  CM_CUDA(cudaMemcpyAsync(out, ctx->d_lev, (size_t)nlev * CM_DG_NPROF * sizeof(double), cudaMemcpyDeviceToHost, ctx->st));
+  CM_CUDA(cudaStreamSynchronize(ctx->st));
   return CM_DG_OK;
 }
 

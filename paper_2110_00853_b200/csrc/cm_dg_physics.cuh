@@ -222,6 +222,27 @@ __device__ __forceinline__ void cm_hllc(const double* Ym, const CmPrim& Pm, cons
   for (int v = 0; v < NV; ++v) Fs[v] = AF[v] + sJ * (SK * dU[v]);
 }
 
+// Surface fluxes of the bottom wall (face 4), added to the wall's lifted flux term r = -sJ n.F* (+ own side):
+//   energy  n_in . rho (J + D) = SHF + LHF (p.shf holds the sum), water and with it mass E = n_in . (rho d_qv)
+//   (P:L672-679), momentum  n_in . (rho tau) = -rho C_d |u_p,int| u_p,int  (eq. A2) with u_p,int the
+//   wall-parallel velocity at the first layer of interior nodes: Yi = state of the node above the wall node (stride si).
+// A = outward sJ n of the wall node, rho = density at the wall node.
+template <bool MOIST>
+__device__ __forceinline__ void cm_surface_flux(const CmKP& p, const double* A, double sJ, double rho, const double* Yi, int si,
+                                                double* r) {
+  r[4] += sJ * p.shf;
+  if (MOIST) { r[0] += sJ * p.evap; r[5] += sJ * p.evap; }
+  if (p.drag_cd > 0.0) {
+    const double ir = cm_rcp(Yi[0]), isJ = cm_rcp(sJ);
+    const double u = Yi[si] * ir, v = Yi[2 * si] * ir, w = Yi[3 * si] * ir;
+    const double n0 = A[0] * isJ, n1 = A[1] * isJ, n2 = A[2] * isJ;
+    const double un = u * n0 + v * n1 + w * n2;
+    const double u0 = u - un * n0, u1 = v - un * n1, u2 = w - un * n2;
+    const double c = sJ * rho * p.drag_cd * cm_sqrt(u0 * u0 + u1 * u1 + u2 * u2);
+    r[1] -= c * u0; r[2] -= c * u1; r[3] -= c * u2;
+  }
+}
+
 template <int NV>
 __device__ __forceinline__ void cm_load_state(const double* __restrict__ Q, long long stride, size_t idx, double* Y) {
 #pragma unroll
