@@ -17,7 +17,7 @@
 //   O10 diagnostics: eq. (57), (61)-(62) P:L587-591
 //   O11 Vreman eddy viscosity (eq. 39a-d) and the Richardson stability factor (eq. 40)
 //   O12 Rayleigh sponge (eq. A4-A5) and the exponential element filter (eq. 52)
-//   O13 any 2N-storage LSRK coefficient table, HLLC flux (named P:L256; Toro et al. 1994, textbook form),
+//   O13 any 2N-storage LSRK coefficient table, HLLC and Roe fluxes (named P:L256; textbook forms),
 //       curl-invariant metric terms (Kopriva 2006) for fully 3-D warps
 //   O14 surface fluxes at the bottom wall: aerodynamic drag law (eq. A2), prescribed evaporation and latent
 //       heat flux; density-weighted horizontal statistics (eq. B1-B4)
@@ -64,7 +64,7 @@ struct Ctx {
   double p_0 = 1.0e5;              // reference pressure of theta_v (R25)
   double sponge_alpha = 0.0, sponge_zs = 0.0; int sponge_gamma = 2; double u_relax[3] = {0, 0, 0};   // eq. (A4)-(A5)
   int filter_order = 0; double filter_alpha = 36.0436533891172;   // eq. (52); alpha = -log(2^-52)
-  int riemann = 0;                 // 0 Rusanov (eq. 27) | 1 HLLC
+  int riemann = 0;                 // 0 Rusanov (eq. 27) | 1 HLLC | 2 Roe
   int metric_form = 0;             // 0 cross-product (R4) | 1 curl-invariant
   double drag_cd = 0.0;            // C_d of the drag law (A2) on the bottom wall, 0 = free slip
   double lhf_bottom = 0.0;         // latent heat flux LHF [W m^-2] added to SHF in the wall energy flux
@@ -470,6 +470,39 @@ void numerical_flux(const Ctx& c, const double* Ym, const Prim& Pm, const double
   if (c.riemann == 0) {
     double lam = std::max(std::fabs(unm) + Pm.c, std::fabs(unp) + Pp.c);   // R2
     for (int v = 0; v < nv; ++v) Fstar[v] = 0.5 * (nFm[v] + nFp[v]) + 0.5 * lam * (Ym[v] - Yp[v]);   // eq. (27), reading R1
+    return;
+  }
+  if (c.riemann == 2) {
+    // Roe (named at P:L256; Roe 1981, textbook form): F* = (1/2)(F^- + F^+) - (1/2) sum_k |lambda_k| alpha_k r_k with the
+    // sqrt(rho)-weighted averages u~, H~ (total enthalpy), q~.  With the mixture frozen at q~ the EOS of eq. (6)-(14) is an
+    // ideal gas with gamma - 1 = kappa~ = R_m / c_vm and the energy shifted by s~ = Phi + q~ I_v0 - c_vm T_0:
+    // p = kappa (rho e - rho |u|^2 / 2 - rho s), hence c~^2 = kappa~ (H~ - s~ - |u~|^2 / 2).  Exact Roe linearisation for dry
+    // air; rho q is a passive wave of speed u~_n (reading R30).  No entropy fix.
+    double wm = std::sqrt(Ym[0]), wp = std::sqrt(Yp[0]), iw = 1.0 / (wm + wp);
+    double ut[3], un = 0, K = 0;
+    for (int i = 0; i < 3; ++i) { ut[i] = (wm * Pm.u[i] + wp * Pp.u[i]) * iw; un += ut[i] * nrm[i]; K += 0.5 * ut[i] * ut[i]; }
+    double H = (wm * Pm.htot + wp * Pp.htot) * iw;
+    double q = (nv == 6) ? (wm * Pm.q + wp * Pp.q) * iw : 0.0;
+    double cvm = c.c_vd * (1.0 - q) + c.c_vv * q, Rm = c.R_d * (1.0 - q) + c.R_v * q;
+    double kappa = Rm / cvm;
+    double sh = Pm.Phi + q * c.I_v0 - cvm * c.T_0;          // Phi is the same on both sides of a face
+    double c2 = kappa * (H - sh - K), cs = std::sqrt(c2);
+    double rt = wm * wp;                                     // rho~
+    double drho = Yp[0] - Ym[0], dp = Pp.pp - Pm.pp, dun = unp - unm;
+    double du[3]; for (int i = 0; i < 3; ++i) du[i] = Pp.u[i] - Pm.u[i];
+    double a1 = (dp - rt * cs * dun) / (2.0 * c2), a5 = (dp + rt * cs * dun) / (2.0 * c2), a2 = drho - dp / c2;
+    double l1 = std::fabs(un - cs), l2 = std::fabs(un), l5 = std::fabs(un + cs);
+    double D[6];
+    D[0] = l1 * a1 + l2 * a2 + l5 * a5;
+    double udu = 0;
+    for (int i = 0; i < 3; ++i) {
+      double sh_i = du[i] - dun * nrm[i];                    // shear part of the velocity jump
+      D[1 + i] = l1 * a1 * (ut[i] - cs * nrm[i]) + l2 * (a2 * ut[i] + rt * sh_i) + l5 * a5 * (ut[i] + cs * nrm[i]);
+      udu += ut[i] * sh_i;
+    }
+    D[4] = l1 * a1 * (H - cs * un) + l2 * (a2 * (K + sh) + rt * udu) + l5 * a5 * (H + cs * un);
+    if (nv == 6) D[5] = (l1 * a1 + l2 * a2 + l5 * a5) * q + l2 * rt * (Pp.q - Pm.q);
+    for (int v = 0; v < nv; ++v) Fstar[v] = 0.5 * (nFm[v] + nFp[v]) - 0.5 * D[v];
     return;
   }
   double SL = std::min(unm - Pm.c, unp - Pp.c), SR = std::max(unm + Pm.c, unp + Pp.c);
