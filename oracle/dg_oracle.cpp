@@ -19,6 +19,8 @@
 //   O12 Rayleigh sponge (eq. A4-A5) and the exponential element filter (eq. 52)
 //   O13 any 2N-storage LSRK coefficient table, HLLC and Roe fluxes (named P:L256; textbook forms),
 //       curl-invariant metric terms (Kopriva 2006) for fully 3-D warps
+//   O15 saturation adjustment (eq. 15): Newton iteration for T with the closed-form saturation vapour pressure
+//       of a calorically perfect gas (Romps 2008, cited P:L172); warm phase (liquid condensate) -- reading R31
 //   O14 surface fluxes at the bottom wall: aerodynamic drag law (eq. A2), prescribed evaporation and latent
 //       heat flux; density-weighted horizontal statistics (eq. B1-B4)
 // Readings of the paper where it is silent or garbled are R1..R29 of DESIGN.md.
@@ -66,6 +68,9 @@ struct Ctx {
   int filter_order = 0; double filter_alpha = 36.0436533891172;   // eq. (52); alpha = -log(2^-52)
   int riemann = 0;                 // 0 Rusanov (eq. 27) | 1 HLLC | 2 Roe
   int metric_form = 0;             // 0 cross-product (R4) | 1 curl-invariant
+  int satadj = 0;                  // 1: temperature and condensate from the saturation adjustment of eq. (15)
+  double c_vl = 4181.0;            // Table 1
+  double p_tr = 611.657, T_tr = 273.16;   // triple point of water (anchor of the saturation vapour pressure, R31)
   double drag_cd = 0.0;            // C_d of the drag law (A2) on the bottom wall, 0 = free slip
   double lhf_bottom = 0.0;         // latent heat flux LHF [W m^-2] added to SHF in the wall energy flux
   double evap_bottom = 0.0;        // evaporation E [kg m^-2 s^-1] into the domain through the bottom wall
@@ -269,8 +274,48 @@ inline int face_node(int Nq, int f, int a, int b, bool other_side) {
 
 // ---------------------------------------------------------------- O3: thermodynamics at a node
 struct Prim {
-  double rho, u[3], q, K, Phi, T, p, pp /* p - p_r */, htot, c, rho_r, theta_v;
+  double rho, u[3], q, K, Phi, T, p, pp /* p - p_r */, htot, c, rho_r, theta_v, ql /* liquid specific humidity */;
 };
+
+// O15.  Saturation vapour pressure over liquid with constant heat capacities (Romps 2008): Clausius-Clapeyron
+//   d ln p* / dT = L(T) / (R_v T^2),  L(T) = L_v0 + (c_pv - c_pl)(T - T_0),  c_pv = c_vv + R_v,  c_pl = c_vl,
+// integrated from the triple point (T_tr, p_tr):
+//   p*(T) = p_tr (T / T_tr)^(dcp / R_v) exp[ ((L_v0 - dcp T_0) / R_v) (1 / T_tr - 1 / T) ],  dcp = c_pv - c_pl.
+double sat_vapor_pressure(const Ctx& c, double T) {
+  double dcp = (c.c_vv + c.R_v) - c.c_vl, Lv0 = c.I_v0 + c.R_v * c.T_0;        // eq. (9)
+  return c.p_tr * std::pow(T / c.T_tr, dcp / c.R_v) * std::exp((Lv0 - dcp * c.T_0) / c.R_v * (1.0 / c.T_tr - 1.0 / T));
+}
+// saturation specific humidity at given density: q_v* = p*(T) / (rho R_v T)
+double sat_q(const Ctx& c, double T, double rho) { return sat_vapor_pressure(c, T) / (rho * c.R_v * T); }
+
+// internal energy at equilibrium I*(T; rho, q_t) of eq. (15) with eq. (7)-(8): unsaturated (q_v = q_t) or saturated with
+// the excess q_t - q_v*(T, rho) as liquid
+double internal_energy_eq(const Ctx& c, double T, double rho, double qt, double* ql_out) {
+  double qvs = sat_q(c, T, rho);
+  double qv = std::min(qt, qvs), ql = qt - qv;
+  if (ql_out) *ql_out = ql;
+  return (1.0 - qt) * c.c_vd * (T - c.T_0) + qv * (c.c_vv * (T - c.T_0) + c.I_v0) + ql * c.c_vl * (T - c.T_0);
+}
+
+// root T of I*(T; rho, q_t) - I = 0 (eq. 15) by Newton iterations with the analytical derivative; ql = condensate
+double saturation_adjustment(const Ctx& c, double I, double rho, double qt, double* ql) {
+  double cvm = c.c_vd * (1.0 - qt) + c.c_vv * qt;
+  double T = c.T_0 + (I - qt * c.I_v0) / cvm;                 // unsaturated: eq. (7)-(8) solved for T
+  if (qt <= sat_q(c, T, rho)) { *ql = 0.0; return T; }
+  double dcp = (c.c_vv + c.R_v) - c.c_vl, Lv0 = c.I_v0 + c.R_v * c.T_0;
+  for (int it = 0; it < 50; ++it) {
+    double qvs = sat_q(c, T, rho);
+    double f = (1.0 - qt) * c.c_vd * (T - c.T_0) + qvs * (c.c_vv * (T - c.T_0) + c.I_v0) + (qt - qvs) * c.c_vl * (T - c.T_0) - I;
+    double L = Lv0 + dcp * (T - c.T_0);
+    double dqvs = qvs * (L / (c.R_v * T * T) - 1.0 / T);      // d q_v* / dT at fixed rho
+    double df = (1.0 - qt) * c.c_vd + qvs * c.c_vv + (qt - qvs) * c.c_vl + dqvs * ((c.c_vv - c.c_vl) * (T - c.T_0) + c.I_v0);
+    double dT = f / df;
+    T -= dT;
+    if (std::fabs(dT) <= 1e-14 * T) break;
+  }
+  *ql = qt - sat_q(c, T, rho);
+  return T;
+}
 
 Prim primitives(const Ctx& c, const double* Y, double z, bool has_ref, double rr, double rer, double rqr) {
   Prim P;
@@ -283,13 +328,26 @@ Prim primitives(const Ctx& c, const double* Y, double z, bool has_ref, double rr
   double cvm = c.c_vd * (1.0 - P.q) + c.c_vv * P.q;                     // eq. (7)-(8), q_v=q_t, q_l=q_i=0
   double Rm = c.R_d * (1.0 - P.q) + c.R_v * P.q;                        // eq. (14)
   P.T = c.T_0 + (eint - P.q * c.I_v0) / cvm;
+  P.ql = 0.0;
+  if (c.satadj && c.nvar == 6) {
+    P.T = saturation_adjustment(c, eint, P.rho, P.q, &P.ql);            // eq. (15)
+    cvm = c.c_vd * (1.0 - P.q) + c.c_vv * (P.q - P.ql) + c.c_vl * P.ql;   // eq. (7)-(8) with condensate
+    Rm = c.R_d * (1.0 - P.q) + c.R_v * (P.q - P.ql);                    // eq. (14): R_d [1 + (eps - 1) q_t - eps q_c]
+  }
   P.p = P.rho * Rm * P.T;                                               // eq. (13)
   P.htot = Y[4] / Y[0] + Rm * P.T;                                      // (rho e + p)/rho
   P.c = std::sqrt((1.0 + Rm / cvm) * Rm * P.T);
   // virtual potential temperature without condensate (R25): theta_v = T (R_m / R_d) (p_0 / p)^(R_d / c_pd)
   P.theta_v = P.T * (Rm / c.R_d) * std::pow(c.p_0 / P.p, c.R_d / (c.c_vd + c.R_d));
   P.rho_r = 0.0;
-  if (has_ref) {
+  if (has_ref && c.satadj && c.nvar == 6) {
+    // with condensate the pressure is no longer linear in the state (R12 does not apply): p_r is the pressure of the
+    // resting reference state under the same equation of state, and p' the plain difference
+    double Yr[6] = {rr, 0.0, 0.0, 0.0, rer, rqr};
+    Prim Pr = primitives(c, Yr, z, false, 0, 0, 0);
+    P.pp = P.p - Pr.p;
+    P.rho_r = rr;
+  } else if (has_ref) {
     // R12: p - p_r evaluated from state differences (exact identity for the EOS above, with
     // p_r := EOS pressure of the resting reference state (rho_r, 0, rhoe_r, rhoq_r)).
     double rq = (c.nvar == 6) ? Y[5] : 0.0;
@@ -853,6 +911,7 @@ struct odg_params {
   int32_t riemann;
   int32_t metric_form;
   double drag_cd, lhf_bottom, evap_bottom;
+  int32_t satadj; double c_vl, p_tr, T_tr;
 };
 
 void odg_lgl(int N, double* xi, double* w) { lgl_nodes_weights(N, xi, w); }
@@ -883,6 +942,10 @@ void* odg_create(const odg_params* p) {
   c->filter_order = p->filter_order; c->filter_alpha = p->filter_alpha;
   c->riemann = p->riemann; c->metric_form = p->metric_form;
   c->drag_cd = p->drag_cd; c->lhf_bottom = p->lhf_bottom; c->evap_bottom = p->evap_bottom;
+  c->satadj = p->satadj;
+  if (p->c_vl > 0.0) c->c_vl = p->c_vl;
+  if (p->p_tr > 0.0) c->p_tr = p->p_tr;
+  if (p->T_tr > 0.0) c->T_tr = p->T_tr;
   lgl_nodes_weights(c->N, c->xi, c->w);
   deriv_matrix(c->N, c->xi, c->D);
   if (c->filter_order > 0) filter_matrix(c->N, c->xi, c->filter_order, c->filter_alpha, c->Filt);
@@ -947,13 +1010,15 @@ void odg_elem_dxd(void* h, int64_t e, double* dxd) {
   for (int n = 0; n < 3 * c.Np; ++n) dxd[n] = g.dxd[n];
 }
 
-// pointwise thermodynamics: out = rho,u,v,w,q,T,p,pp,htot,c,theta_v
+// pointwise thermodynamics: out = rho,u,v,w,q,T,p,pp,htot,c,theta_v,q_l
 void odg_primitives(void* h, const double* Y, double z, int has_ref, double rr, double rer, double rqr, double* out) {
   const Ctx& c = *(Ctx*)h;
   Prim P = primitives(c, Y, z, has_ref != 0, rr, rer, rqr);
   out[0] = P.rho; out[1] = P.u[0]; out[2] = P.u[1]; out[3] = P.u[2]; out[4] = P.q; out[5] = P.T; out[6] = P.p;
-  out[7] = P.pp; out[8] = P.htot; out[9] = P.c; out[10] = P.theta_v;
+  out[7] = P.pp; out[8] = P.htot; out[9] = P.c; out[10] = P.theta_v; out[11] = P.ql;
 }
+// saturation vapour pressure over liquid [Pa] (O15)
+double odg_sat_vapor_pressure(void* h, double T) { return sat_vapor_pressure(*(Ctx*)h, T); }
 
 // pointwise Rusanov flux n.F1* of two states at height z without reference state (pins: consistency, symmetry)
 void odg_rusanov(void* h, const double* Ym, const double* Yp, const double* nrm, double z, double* Fstar) {

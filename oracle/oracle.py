@@ -40,6 +40,7 @@ class _Params(C.Structure):
         ("sponge_alpha", C.c_double), ("sponge_zs", C.c_double), ("sponge_gamma", C.c_int32), ("u_relax", C.c_double * 3),
         ("filter_order", C.c_int32), ("filter_alpha", C.c_double), ("riemann", C.c_int32), ("metric_form", C.c_int32),
         ("drag_cd", C.c_double), ("lhf_bottom", C.c_double), ("evap_bottom", C.c_double),
+        ("satadj", C.c_int32), ("c_vl", C.c_double), ("p_tr", C.c_double), ("T_tr", C.c_double),
     ]
 
 
@@ -62,6 +63,8 @@ def lib():
         L.odg_neighbour.restype = C.c_int64
         L.odg_neighbour.argtypes = [C.c_void_p, C.c_int64, C.c_int]
         L.odg_num_threads.restype = C.c_int
+        L.odg_sat_vapor_pressure.restype = C.c_double
+        L.odg_sat_vapor_pressure.argtypes = [C.c_void_p, C.c_double]
         for name, args in {
             "odg_lgl": [C.c_int, _dp, _dp],
             "odg_dmat": [C.c_int, _dp],
@@ -170,6 +173,8 @@ class Oracle:
         p.riemann = int(cfg.get("riemann", 0)); p.metric_form = int(cfg.get("metric_form", 0))
         p.drag_cd = float(cfg.get("drag_cd", 0.0)); p.lhf_bottom = float(cfg.get("lhf_bottom", 0.0))
         p.evap_bottom = float(cfg.get("evap_bottom", 0.0))
+        p.satadj = int(cfg.get("satadj", 0)); p.c_vl = float(cfg.get("c_vl", 0.0))
+        p.p_tr = float(cfg.get("p_tr", 0.0)); p.T_tr = float(cfg.get("T_tr", 0.0))
         self._h = L.odg_create(C.byref(p))
         if not self._h:
             raise ValueError("odg_create rejected the parameters")
@@ -208,12 +213,15 @@ class Oracle:
 
     # ---- pointwise
     def primitives(self, Y, z=0.0, ref=None):
-        Y = np.ascontiguousarray(Y, dtype=np.float64); out = np.zeros(11)
+        Y = np.ascontiguousarray(Y, dtype=np.float64); out = np.zeros(12)
         if ref is None:
             lib().odg_primitives(self._h, _ptr(Y), float(z), 0, 0.0, 0.0, 0.0, _ptr(out))
         else:
             lib().odg_primitives(self._h, _ptr(Y), float(z), 1, float(ref[0]), float(ref[1]), float(ref[2]), _ptr(out))
-        return dict(zip(("rho", "u", "v", "w", "q", "T", "p", "pp", "htot", "c", "theta_v"), out))
+        return dict(zip(("rho", "u", "v", "w", "q", "T", "p", "pp", "htot", "c", "theta_v", "ql"), out))
+
+    def sat_vapor_pressure(self, T):
+        return float(lib().odg_sat_vapor_pressure(self._h, float(T)))
 
     def rusanov(self, Ym, Yp, n, z=0.0):
         Ym = np.ascontiguousarray(Ym, dtype=np.float64); Yp = np.ascontiguousarray(Yp, dtype=np.float64)
