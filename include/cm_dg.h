@@ -72,8 +72,8 @@ typedef struct {
   int32_t filter_order;     /* exponential element filter of eq. (52): order s (even, e.g. 64), 0 = off;
                                when on, cm_dg_lsrk_step* apply it after every time step (cm_dg_filter applies it once) */
   double filter_alpha;      /* alpha = -log(eps_M) of eq. (52); 0 = 36.0436533891172 (double precision)       */
-  int32_t riemann;          /* numerical flux of F1: 0 Rusanov (eq. 27) | 1 HLLC; HLLC runs on the
-                               stored-metric kernels                                                          */
+  int32_t riemann;          /* numerical flux of F1: 0 Rusanov (eq. 27) | 1 HLLC | 2 Roe (both named at P:L256); HLLC and
+                               Roe run on the stored-metric kernels                                           */
   int32_t metric_form;      /* 0 cross-product metric terms (extruded / 2.5-D warps) | 1 curl-invariant form
                                (fully 3-D warps; geom == 2)                                                   */
   /* ---- surface fluxes through the z-low wall (App. A1; need bc[2] == 1); all-zero = free slip, no flux ---- */
@@ -82,6 +82,13 @@ typedef struct {
   double lhf_bottom;        /* W m^-2 latent heat flux, added to shf_bottom in the wall energy flux   */
   double evap_bottom;       /* kg m^-2 s^-1 evaporation E = n.(rho d_qv)|sfc into the domain: enters the
                                rho*q_tot and rho equations (nvar == 6); the caller derives it from LHF                */
+  /* ---- equilibrium moist thermodynamics (section 2.7, eq. 15); nvar == 6; runs on the stored-metric kernels ---- */
+  int32_t satadj;           /* 1: temperature and liquid water from the saturation adjustment: the root T of
+                               I*(T; rho, q_tot) = I by Newton iterations, the saturation excess q_tot - q_v*(T, rho) as liquid
+                               (warm phase), q_v* from the closed-form saturation vapour pressure of a calorically perfect gas
+                               (Romps 2008); R_m, c_vm, p and the sound speed then include the condensate (eq. 7-8, 13-14)   */
+  double c_vl;              /* isochoric heat capacity of liquid water (Table 1); 0 = 4181 J/(kg K)              */
+  double p_triple, T_triple;/* triple point of water anchoring p*(T); 0 = 611.657 Pa, 273.16 K                               */
 } cm_dg_params;
 
 /* Optional scheduling knobs (HOST, copied by cm_dg_setup_tuned).  They never change what is computed (the parity tests

@@ -27,6 +27,7 @@ class _Params(C.Structure):
         ("sponge_alpha", C.c_double), ("sponge_zs", C.c_double), ("sponge_gamma", C.c_int32), ("u_relax", C.c_double * 3),
         ("filter_order", C.c_int32), ("filter_alpha", C.c_double), ("riemann", C.c_int32), ("metric_form", C.c_int32),
         ("drag_cd", C.c_double), ("lhf_bottom", C.c_double), ("evap_bottom", C.c_double),
+        ("satadj", C.c_int32), ("c_vl", C.c_double), ("p_triple", C.c_double), ("T_triple", C.c_double),
     ]
 
 
@@ -147,11 +148,12 @@ def cm_dg_setup(cfg, stream=None, tuning=None):
     for k in ("R_d", "c_vd", "R_v", "c_vv", "T_0", "I_v0", "grav", "C_s", "Pr_t", "shf_bottom"):
         setattr(p, k, float(cfg[k]))
     p.sgs = int(cfg.get("sgs", 0))
-    for k in ("richardson", "sponge_gamma", "filter_order", "riemann", "metric_form"):
+    for k in ("richardson", "sponge_gamma", "filter_order", "riemann", "metric_form", "satadj"):
         setattr(p, k, int(cfg.get(k, 0)))
-    for k in ("p_0", "sponge_alpha", "sponge_zs", "filter_alpha", "drag_cd", "lhf_bottom", "evap_bottom"):
+    for k in ("p_0", "sponge_alpha", "sponge_zs", "filter_alpha", "drag_cd", "lhf_bottom", "evap_bottom", "c_vl"):
         setattr(p, k, float(cfg.get(k, 0.0)))
     p.u_relax[:] = [float(v) for v in cfg.get("u_relax", (0.0, 0.0, 0.0))]
+    p.p_triple = float(cfg.get("p_tr", 0.0)); p.T_triple = float(cfg.get("T_tr", 0.0))
     p.use_ref = int(cfg.get("use_ref", 0))
     if p.use_ref:
         p.ref_rho = host("ref_rho"); p.ref_rhoe = host("ref_rhoe"); p.ref_rhoq = host("ref_rhoq")

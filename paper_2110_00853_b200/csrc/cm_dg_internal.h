@@ -17,6 +17,9 @@ struct CmThermo {
   double dk;   // a c_vd - R_d b   (numerator of kappa - kappa_r, reading R12)
   double icvd, kappa_d;  // 1 / c_vd, R_d / c_vd (dry air)
   double p_0, kap_pd, iRd;   // theta_v = (p / (rho R_d)) (p_0 / p)^(R_d / c_pd)   (eq. 40, reading R25)
+  // saturation adjustment (eq. 15; stored-metric kernels): p*(T) = p_tr (T / T_tr)^sx1 exp(sx2 (1 / T_tr - 1 / T))
+  double R_v, c_vv, c_vl, Lv0, dcp;   // L(T) = Lv0 + dcp (T - T_0), dcp = c_vv + R_v - c_vl
+  double p_tr, iT_tr, sx1, sx2;       // sx1 = dcp / R_v, sx2 = (Lv0 - dcp T_0) / R_v
 };
 
 // Kernel argument block (passed by value, lives in the constant bank).
@@ -32,8 +35,9 @@ struct CmKP {
   long long stride;      // field stride in doubles
   int sgs;               // 0 inviscid | 1 Smagorinsky-Lilly | 2 Vreman
   int richardson;        // eq. (40): nu_t *= f_b (one more gradient variable, theta_v)
-  int riemann;           // 0 Rusanov | 1 HLLC (stored-metric kernels)
+  int riemann;           // 0 Rusanov | 1 HLLC | 2 Roe (stored-metric kernels)
   int use_ref;           // reference state removed (R12) or plain pressure
+  int satadj;            // 1: temperature and liquid water from the saturation adjustment of eq. (15) (stored-metric kernels)
   int mode;              // tendency: 0 dQ := rhs | 1 LSRK stage.  gradient: 0 packed SGS fluxes | 1 raw 15 gradients
   // arrays
   const double* Q;       // [nvar][stride]

@@ -21,7 +21,35 @@ template <int Nq> struct CmCfg2 {
   static constexpr int EPB = (Nq <= 3) ? 8 : (Nq == 4) ? 4 : (Nq == 5) ? 2 : 1;
   static constexpr int THREADS = EPB * TPE;
   static constexpr int MINB = (Nq <= 5) ? 3 : (Nq == 6) ? 3 : (Nq == 7) ? 2 : 1;   // CTAs per SM the register budget aims at
+#ifndef CM_2_MINB_T
+#define CM_2_MINB_T MINB
+#endif
+  static constexpr int MINB_T = CM_2_MINB_T;       // same for the tendency kernel
 };
+
+// L2 prefetch of the n doubles at a (cp.async.bulk.prefetch.L2 wants a 16-byte aligned address and size; the state arrays
+// are padded by one double, so rounding outwards stays inside them)
+__device__ __forceinline__ void cm2_prefetch_tile(const double* a, int n) {
+  const unsigned long long lo = (unsigned long long)a & ~15ull, hi = ((unsigned long long)(a + n) + 15ull) & ~15ull;
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(lo), "r"((unsigned)(hi - lo)) : "memory");
+}
+// every array the kernels will read for element ea (one wave of resident CTAs further on in the launch order) into L2, one
+// tile per thread t: the loads of that CTA then wait on L2, not on DRAM
+template <int NP, int GEOM>
+__device__ __forceinline__ void cm2_prefetch_element(const CmKP& p, int ea, int t, int nv, bool with_g, int ng, bool with_res) {
+  if (ea >= p.Ne) return;
+  const size_t off = (size_t)ea * NP;
+  int k = t;
+  if (k < nv) { cm2_prefetch_tile(p.Q + (size_t)k * p.stride + off, NP); return; }
+  k -= nv;
+  if (with_g) { if (k < ng) { cm2_prefetch_tile(p.G + (size_t)k * p.stride + off, NP); return; } k -= ng; }
+  if (with_res) { if (k < nv) { cm2_prefetch_tile(p.dQ + (size_t)k * p.stride + off, NP); return; } k -= nv; }
+  if (GEOM != 0) {
+    if (k < CM_NGEO) { cm2_prefetch_tile(p.geo + (size_t)k * p.stride + off, NP); return; }
+    k -= CM_NGEO;
+    if (p.use_ref && k < 3 && (k < 2 || nv == 6)) cm2_prefetch_tile(p.ref + (size_t)k * p.stride + off, NP);
+  }
+}
 
 // node indices of face task (f, a, b): own node nm, coincident node np_ of the neighbour, their zeta indices
 template <int Nq>
@@ -38,7 +66,7 @@ __device__ __forceinline__ void cm2_face_nodes(int f, int a, int b, int& nm, int
 // a2: auxiliary gradient + Smagorinsky-Lilly, thread per node
 // ------------------------------------------------------------------------------------------------
 // RICH: theta_v is a further gradient variable (eq. 40)
-template <int Nq, bool MOIST, int GEOM, bool RICH = false>
+template <int Nq, bool MOIST, int GEOM, bool RICH = false, bool SAT = false>
 __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_gradient_kernel(const __grid_constant__ CmKP p) {
   using C = CmCfg2<Nq>;
   constexpr int NF = C::NF, NP = C::NP, N = Nq - 1, TPE = C::TPE, EPB = C::EPB;
@@ -55,12 +83,13 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_gra
   const int e0 = blockIdx.x * EPB;
   const int e = e0 + el;
   const bool active = e < p.Ne;
+  if (p.ahead > 0 && active) cm2_prefetch_element<NP, GEOM>(p, e + p.ahead, t, NV, false, 0, false);
 
   if (active && t < NP) {
     double Y[6]; CmSite st; CmPrim P;
     cm_load_state<NV>(p.Q, p.stride, (size_t)e * NP + t, Y);
     cm_load_site<Nq, MOIST, GEOM>(p, e, t, t / NF, st);
-    cm_eos<MOIST>(p, Y, st, P);
+    cm_eos<MOIST, SAT>(p, Y, st, P);
     double* s = s_sh + (size_t)el * NS * NP + t;
     s[0] = P.u; s[NP] = P.v; s[2 * NP] = P.w; s[3 * NP] = P.h;
     if (MOIST) s[4 * NP] = P.q;
@@ -109,7 +138,7 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_gra
         double Y[6]; CmSite st; CmPrim P;
         cm_load_state<NV>(p.Q, p.stride, (size_t)nb * NP + np_, Y);
         cm_load_site<Nq, MOIST, GEOM>(p, nb, np_, kp, st);
-        cm_eos<MOIST>(p, Y, st, P);
+        cm_eos<MOIST, SAT>(p, Y, st, P);
         delta[0] = 0.5 * (P.u - sm[0]); delta[1] = 0.5 * (P.v - sm[1]); delta[2] = 0.5 * (P.w - sm[2]);
         delta[3] = 0.5 * (P.h - sm[3]);
         if (MOIST) delta[4] = 0.5 * (P.q - sm[4]);
@@ -189,8 +218,8 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_gra
 // ------------------------------------------------------------------------------------------------
 // a3-a5: tendency + fused LSRK update, thread per node
 // ------------------------------------------------------------------------------------------------
-template <int Nq, bool MOIST, int GEOM>
-__global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_tendency_kernel(const __grid_constant__ CmKP p) {
+template <int Nq, bool MOIST, int GEOM, bool SAT = false>
+__global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB_T) cm2_tendency_kernel(const __grid_constant__ CmKP p) {
   using C = CmCfg2<Nq>;
   constexpr int NF = C::NF, NP = C::NP, N = Nq - 1, TPE = C::TPE, EPB = C::EPB;
   constexpr int NV = MOIST ? 6 : 5;
@@ -206,6 +235,7 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_ten
   const int e0 = blockIdx.x * EPB;
   const int e = e0 + el;
   const bool active = e < p.Ne;
+  if (p.ahead > 0 && active) cm2_prefetch_element<NP, GEOM>(p, e + p.ahead, t, NV, p.sgs != 0, NG, p.mode == 1 && p.rka != 0.0);
   double buoy = 0.0, taus = 0.0;
 
   // ---- phase 0: primitives and fluxes of the own node -> shared memory
@@ -215,7 +245,7 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_ten
     cm_load_state<NV>(p.Q, p.stride, idx, Y);
     if (p.sgs) cm_load_state<NG>(p.G, p.stride, idx, g);
     cm_load_site<Nq, MOIST, GEOM>(p, e, t, t / NF, st);
-    cm_eos<MOIST>(p, Y, st, P);
+    cm_eos<MOIST, SAT>(p, Y, st, P);
     buoy = P.drho * p.th.grav; taus = st.taus;
     double* q = Q_sh + (size_t)el * NV * NP + t;
 #pragma unroll
@@ -289,7 +319,7 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_ten
           cm_load_state<NV>(p.Q, p.stride, idp, Yp);
           if (p.sgs) cm_load_state<NG>(p.G, p.stride, idp, g);
           cm_load_site<Nq, MOIST, GEOM>(p, nb, np_, kp, st);
-          cm_eos<MOIST>(p, Yp, st, P);
+          cm_eos<MOIST, SAT>(p, Yp, st, P);
           cm_flux_dir<MOIST>(Yp, P, p.sgs, g, A[0], A[1], A[2], Fp);
           c2p = P.c2;
           uAp = A[0] * P.u + A[1] * P.v + A[2] * P.w;
@@ -299,12 +329,13 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_ten
 #pragma unroll
           for (int v = 0; v < NV; ++v) r[v] = 0.5 * (Ftm[v] - Fp[v]) - 0.5 * lamsJ * (Ym[v] - Yp[v]);
         } else {
-          // HLLC for F1, central flux for F2: sJ F* = Fs + (1/2)(Ftm - A.F1^-) + (1/2)(Fp - A.F1^+)
+          // HLLC or Roe for F1, central flux for F2: sJ F* = Fs + (1/2)(Ftm - A.F1^-) + (1/2)(Fp - A.F1^+)
           CmSite sm_, sp_; CmPrim Pm, Pp; double AFm[6], AFp[6], Fs[6];
-          cm_load_site<Nq, MOIST, GEOM>(p, e, nm, km, sm_); cm_eos<MOIST>(p, Ym, sm_, Pm);
-          cm_load_site<Nq, MOIST, GEOM>(p, nb, np_, kp, sp_); cm_eos<MOIST>(p, Yp, sp_, Pp);
+          cm_load_site<Nq, MOIST, GEOM>(p, e, nm, km, sm_); cm_eos<MOIST, SAT>(p, Ym, sm_, Pm);
+          cm_load_site<Nq, MOIST, GEOM>(p, nb, np_, kp, sp_); cm_eos<MOIST, SAT>(p, Yp, sp_, Pp);
           cm_flux1_dir<MOIST>(Ym, Pm, A[0], A[1], A[2], AFm); cm_flux1_dir<MOIST>(Yp, Pp, A[0], A[1], A[2], AFp);
-          cm_hllc<MOIST>(Ym, Pm, AFm, Yp, Pp, AFp, A, sJ, Fs);
+          if (p.riemann == 1) cm_hllc<MOIST>(Ym, Pm, AFm, Yp, Pp, AFp, A, sJ, Fs);
+          else cm_roe<MOIST>(p, Ym, Pm, AFm, Yp, Pp, AFp, A, sJ, sm_.Phi, Fs);
 #pragma unroll
           for (int v = 0; v < NV; ++v) r[v] = Ftm[v] - (Fs[v] + 0.5 * (Ftm[v] - AFm[v]) + 0.5 * (Fp[v] - AFp[v]));
         }
@@ -313,7 +344,7 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_ten
         // second-order normal fluxes vanish (R10) except the prescribed bottom energy flux
         CmSite st; CmPrim P;
         cm_load_site<Nq, MOIST, GEOM>(p, e, nm, km, st);
-        cm_eos<MOIST>(p, Ym, st, P);
+        cm_eos<MOIST, SAT>(p, Ym, st, P);
         const double un = uAm / sJ;
         if (p.riemann == 0) {
           const double lam = fabs(un) + cm_;
@@ -322,7 +353,7 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_ten
           for (int v = 0; v < NV; ++v) r[v] = Ftm[v];
           r[1] -= mom * A[0]; r[2] -= mom * A[1]; r[3] -= mom * A[2];
         } else {
-          // HLLC against the mirrored state (A6)-(A7); n.F2* = 0 at the wall (R10)
+          // HLLC / Roe against the mirrored state (A6)-(A7); n.F2* = 0 at the wall (R10)
           double Yg[6], AFm[6], AFg[6], Fs[6];
           const double mn = 2.0 * (Ym[1] * A[0] + Ym[2] * A[1] + Ym[3] * A[2]) / (sJ * sJ);
 #pragma unroll
@@ -331,7 +362,8 @@ __global__ void __launch_bounds__(CmCfg2<Nq>::THREADS, CmCfg2<Nq>::MINB) cm2_ten
           CmPrim Pg = P;
           Pg.u = Yg[1] * P.ir; Pg.v = Yg[2] * P.ir; Pg.w = Yg[3] * P.ir;
           cm_flux1_dir<MOIST>(Ym, P, A[0], A[1], A[2], AFm); cm_flux1_dir<MOIST>(Yg, Pg, A[0], A[1], A[2], AFg);
-          cm_hllc<MOIST>(Ym, P, AFm, Yg, Pg, AFg, A, sJ, Fs);
+          if (p.riemann == 1) cm_hllc<MOIST>(Ym, P, AFm, Yg, Pg, AFg, A, sJ, Fs);
+          else cm_roe<MOIST>(p, Ym, P, AFm, Yg, Pg, AFg, A, sJ, st.Phi, Fs);
 #pragma unroll
           for (int v = 0; v < NV; ++v) r[v] = Ftm[v] - Fs[v];
         }

@@ -58,33 +58,43 @@ cudaError_t configure(K kernel, size_t smem, LaunchState& ls, int threads = 0, i
   return cudaSuccess;
 }
 
-template <int Nq, bool MOIST, int GEOM, bool RICH>
+template <int Nq, bool MOIST, int GEOM, bool RICH, bool SAT = false>
 cudaError_t launch_grad2r(const CmKP& kp, cudaStream_t st) {
   using C = CmCfg2<Nq>;
   static LaunchState ls;
   constexpr size_t smem = grad2_smem<Nq, MOIST, RICH>();
-  cudaError_t err = configure(cm2_gradient_kernel<Nq, MOIST, GEOM, RICH>, smem, ls);
+  int wave = 0;
+  cudaError_t err = configure(cm2_gradient_kernel<Nq, MOIST, GEOM, RICH, SAT>, smem, ls, C::THREADS, &wave);
   if (err != cudaSuccess) return err;
   const int blocks = (kp.Ne + C::EPB - 1) / C::EPB;
-  cm2_gradient_kernel<Nq, MOIST, GEOM, RICH><<<blocks, C::THREADS, smem, st>>>(kp);
+  CmKP k2 = kp;
+  if (k2.ahead < 0) k2.ahead = wave * C::EPB;   // L2 prefetch distance in elements: one wave of resident CTAs
+  cm2_gradient_kernel<Nq, MOIST, GEOM, RICH, SAT><<<blocks, C::THREADS, smem, st>>>(k2);
   return cudaGetLastError();
 }
 template <int Nq, bool MOIST, int GEOM>
 cudaError_t launch_grad2(const CmKP& kp, cudaStream_t st) {
   // the Richardson factor (eq. 40) needs theta_v as a further gradient variable; the raw-gradient mode does not
+  if constexpr (MOIST) {   // saturation-adjusted equation of state (eq. 15): its own instantiations
+    if (kp.satadj) return (kp.richardson && kp.mode == 0) ? launch_grad2r<Nq, MOIST, GEOM, true, true>(kp, st) : launch_grad2r<Nq, MOIST, GEOM, false, true>(kp, st);
+  }
   if (kp.richardson && kp.mode == 0) return launch_grad2r<Nq, MOIST, GEOM, true>(kp, st);
   return launch_grad2r<Nq, MOIST, GEOM, false>(kp, st);
 }
 
-template <int Nq, bool MOIST, int GEOM>
+template <int Nq, bool MOIST, int GEOM, bool SAT = false>
 cudaError_t launch_tend2(const CmKP& kp, cudaStream_t st) {
   using C = CmCfg2<Nq>;
+  if constexpr (MOIST && !SAT) { if (kp.satadj) return launch_tend2<Nq, MOIST, GEOM, true>(kp, st); }
   static LaunchState ls;
   constexpr size_t smem = tend2_smem<Nq, MOIST>();
-  cudaError_t err = configure(cm2_tendency_kernel<Nq, MOIST, GEOM>, smem, ls);
+  int wave = 0;
+  cudaError_t err = configure(cm2_tendency_kernel<Nq, MOIST, GEOM, SAT>, smem, ls, C::THREADS, &wave);
   if (err != cudaSuccess) return err;
   const int blocks = (kp.Ne + C::EPB - 1) / C::EPB;
-  cm2_tendency_kernel<Nq, MOIST, GEOM><<<blocks, C::THREADS, smem, st>>>(kp);
+  CmKP k2 = kp;
+  if (k2.ahead < 0) k2.ahead = wave * C::EPB;   // L2 prefetch distance in elements: one wave of resident CTAs
+  cm2_tendency_kernel<Nq, MOIST, GEOM, SAT><<<blocks, C::THREADS, smem, st>>>(k2);
   return cudaGetLastError();
 }
 

@@ -14,6 +14,7 @@
 
 #include "../../include/cm_dg.h"
 #include "cm_dg_internal.h"
+#include "cm_dg_physics.cuh"
 
 namespace {
 
@@ -278,7 +279,7 @@ __global__ void general_metrics_copy(long long n, long long stride, const double
 
 // a6: per-block partial sums {mass, energy, water, M |u|^2 / 2, M, max(|u|+c), nonfinite}
 struct DiagArgs {
-  int Nq, Np, nvar, general, use_ref;
+  int Nq, Np, nvar, general, use_ref, satadj;
   long long Ne, stride;
   const double* Q; const double* geo; const int* erow; const double* ztab;
   double Jflat; double w[CM_MAXNQ];
@@ -300,9 +301,10 @@ __global__ void diag_kernel(const __grid_constant__ DiagArgs a, double* __restri
     const double ir = 1.0 / Y[0];
     const double u2 = (Y[1] * Y[1] + Y[2] * Y[2] + Y[3] * Y[3]) * ir * ir;
     const double q = (a.nvar == 6) ? Y[5] * ir : 0.0;
-    const double cvm = a.th.c_vd + a.th.b * q, Rm = a.th.R_d + a.th.a * q;
+    double cvm = a.th.c_vd + a.th.b * q, Rm = a.th.R_d + a.th.a * q;
     const double eint = Y[4] * ir - 0.5 * u2 - Phi;
-    const double T = a.th.T_0 + (eint - q * a.th.I_v0) / cvm;
+    double T = a.th.T_0 + (eint - q * a.th.I_v0) / cvm;
+    if (a.satadj) T = cm_sat_pressure(a.th, Y[0], eint, q, Rm, cvm) / (Y[0] * Rm);
     const double c = sqrt((1.0 + Rm / cvm) * Rm * T);
     s[0] += M * Y[0]; s[1] += M * Y[4]; s[2] += M * Y[5]; s[3] += M * 0.5 * u2; s[4] += M;
     s[5] = fmax(s[5], sqrt(u2) + c);
@@ -388,7 +390,7 @@ __global__ void diag_reduce_kernel(long long Ne, const double* __restrict__ part
 // App. B statistics (eq. B1-B4).  pass 0: per element and nodal zeta-plane the sums of W [1, z, rho, rho phi_m];
 // pass 1: of W rho [w' phi'_m, phi'_m^2] with the level means of pass 0.  W = w_i w_j |Ja^3|.
 struct ProfArgs {
-  int Nq, Np, nvar, general, pass;
+  int Nq, Np, nvar, general, pass, satadj;
   long long Ne, stride;
   const double* Q; const double* geo; const int* erow; const double* ztab;
   const double* lev;                 // pass 1: [nlev][CM_DG_NPROF] level means
@@ -405,7 +407,8 @@ __device__ inline void prof_vars(const ProfArgs& a, const double* Y, double Phi,
   const double K = 0.5 * (Y[1] * u + Y[2] * v + Y[3] * w);
   const double kappa = (th.R_d + th.a * q) / (th.c_vd + th.b * q);
   const double E = Y[4] - K - Y[0] * Phi - rq * th.I_v0;
-  const double pr = kappa * E + th.T_0 * (th.R_d * Y[0] + th.a * rq);
+  double pr = kappa * E + th.T_0 * (th.R_d * Y[0] + th.a * rq);
+  if (a.satadj) { double Rm, cvm; pr = cm_sat_pressure(th, Y[0], (Y[4] - K) * ir - Phi, q, Rm, cvm); }
   phi[0] = u; phi[1] = v; phi[2] = w; phi[3] = (Y[4] + pr) * ir; phi[4] = q;
   phi[5] = pr * ir * th.iRd * pow(th.p_0 / pr, th.kap_pd);          // theta_v without condensate (R25)
 }
@@ -635,12 +638,15 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   if (p->richardson != 0 && p->richardson != 1) return fail(CM_DG_EINVAL, "cm_dg_setup: richardson must be 0 or 1");
   if (p->richardson && !p->sgs) return fail(CM_DG_EINVAL, "cm_dg_setup: richardson = 1 needs an eddy-viscosity closure (sgs != 0)");
   if (p->p_0 < 0.0) return fail(CM_DG_EINVAL, "cm_dg_setup: p_0 must be positive (0 = 1e5 Pa)");
-  if (p->riemann != 0 && p->riemann != 1) return fail(CM_DG_EINVAL, "cm_dg_setup: riemann must be 0 (Rusanov) or 1 (HLLC)");
+  if (p->riemann < 0 || p->riemann > 2) return fail(CM_DG_EINVAL, "cm_dg_setup: riemann must be 0 (Rusanov), 1 (HLLC) or 2 (Roe)");
   if (p->metric_form != 0 && p->metric_form != 1) return fail(CM_DG_EINVAL, "cm_dg_setup: metric_form must be 0 or 1");
   if (p->filter_order < 0 || p->filter_alpha < 0.0) return fail(CM_DG_EINVAL, "cm_dg_setup: filter_order and filter_alpha must be >= 0");
   if (p->sponge_alpha < 0.0 || p->sponge_gamma < 0) return fail(CM_DG_EINVAL, "cm_dg_setup: sponge_alpha and sponge_gamma must be >= 0");
   if (p->sponge_alpha > 0.0 && !(p->sponge_zs < p->hi[2])) return fail(CM_DG_EINVAL, "cm_dg_setup: the sponge must start below hi[2]");
   if (!(p->c_vd > 0.0) || !(p->R_d > 0.0)) return fail(CM_DG_EINVAL, "cm_dg_setup: R_d and c_vd must be positive");
+  if (p->satadj != 0 && p->satadj != 1) return fail(CM_DG_EINVAL, "cm_dg_setup: satadj must be 0 or 1");
+  if (p->satadj && p->nvar != 6) return fail(CM_DG_EINVAL, "cm_dg_setup: satadj = 1 needs the moisture tracer (nvar == 6)");
+  if (p->c_vl < 0.0 || p->p_triple < 0.0 || p->T_triple < 0.0) return fail(CM_DG_EINVAL, "cm_dg_setup: c_vl, p_triple, T_triple must be >= 0");
   if (p->drag_cd < 0.0) return fail(CM_DG_EINVAL, "cm_dg_setup: drag_cd must be >= 0");
   if ((p->drag_cd != 0.0 || p->lhf_bottom != 0.0 || p->evap_bottom != 0.0) && p->bc[2] != 1)
     return fail(CM_DG_EINVAL, "cm_dg_setup: surface fluxes (drag_cd, lhf_bottom, evap_bottom) need a wall in z (bc[2] == 1)");
@@ -733,7 +739,7 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   if (c->general) c->variant = 2;
   // HLLC is implemented in the thread-per-node kernels; so is the Richardson factor at the orders whose flat gradient
   // kernel is the trace-buffer one (N <= 3)
-  if (p->riemann != 0 || (p->richardson && Nq <= 4)) c->variant = 2;
+  if (p->riemann != 0 || p->satadj || (p->richardson && Nq <= 4)) c->variant = 2;
 
   auto bail = [&](int code) { free_ctx(c); return code; };
 #define CM_CUDA_B(call)                                                                                   \
@@ -793,6 +799,16 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   kp.th.T_0 = p->T_0; kp.th.I_v0 = p->I_v0; kp.th.grav = p->grav;
   kp.th.dk = kp.th.a * p->c_vd - p->R_d * kp.th.b;
   kp.th.icvd = 1.0 / p->c_vd; kp.th.kappa_d = p->R_d / p->c_vd;
+  {
+    const double c_vl = p->c_vl > 0.0 ? p->c_vl : 4181.0, p_tr = p->p_triple > 0.0 ? p->p_triple : 611.657;
+    const double T_tr = p->T_triple > 0.0 ? p->T_triple : 273.16;
+    kp.satadj = p->satadj;
+    kp.th.R_v = p->R_v; kp.th.c_vv = p->c_vv; kp.th.c_vl = c_vl;
+    kp.th.Lv0 = p->I_v0 + p->R_v * p->T_0;                                 // eq. (9)
+    kp.th.dcp = p->c_vv + p->R_v - c_vl;
+    kp.th.p_tr = p_tr; kp.th.iT_tr = 1.0 / T_tr;
+    kp.th.sx1 = kp.th.dcp / p->R_v; kp.th.sx2 = (kp.th.Lv0 - kp.th.dcp * p->T_0) / p->R_v;
+  }
   kp.cA[0] = c->h[1] * c->h[2] / 4.0; kp.cA[1] = c->h[0] * c->h[2] / 4.0; kp.cA[2] = c->h[0] * c->h[1] / 4.0;
   kp.invJ = 8.0 / (c->h[0] * c->h[1] * c->h[2]);
   {
@@ -998,7 +1014,7 @@ int cm_dg_diagnostics(cm_dg_ctx* ctx, const double* Q_dev, cm_dg_diag* out) {
   a.Nq = ctx->Nq; a.Np = ctx->Np; a.nvar = ctx->nvar; a.general = ctx->general; a.use_ref = ctx->prm.use_ref;
   a.Ne = ctx->Ne; a.stride = ctx->stride; a.Q = Q_dev; a.geo = ctx->d_geo; a.erow = ctx->d_erow; a.ztab = ctx->d_ztab;
   a.Jflat = 1.0 / ctx->kp.invJ; for (int i = 0; i < CM_MAXNQ; ++i) a.w[i] = ctx->w[i];
-  a.th = ctx->kp.th;
+  a.th = ctx->kp.th; a.satadj = ctx->kp.satadj;
   const int thr = 128;
   {
     Timed tm(ctx, 2);
@@ -1029,7 +1045,7 @@ int cm_dg_profiles(cm_dg_ctx* ctx, const double* Q_dev, double* out, int32_t nle
   a.Ne = ctx->Ne; a.stride = ctx->stride; a.Q = Q_dev; a.geo = ctx->d_geo; a.erow = ctx->d_erow; a.ztab = ctx->d_ztab;
   a.lev = ctx->d_lev; a.A3flat = ctx->kp.cA[2]; a.grav = ctx->prm.grav;
   for (int i = 0; i < CM_MAXNQ; ++i) a.w[i] = ctx->w[i];
-  a.th = ctx->kp.th;
+  a.th = ctx->kp.th; a.satadj = ctx->kp.satadj;
   ProfRedArgs r;
   r.Nq = ctx->Nq; r.Ex = ctx->prm.ne[0]; r.Ey = ctx->prm.ne[1]; r.Ez = ctx->prm.ne[2];
   r.L = ctx->tileL; r.PY = ctx->tilePY; r.NXC = r.Ex / r.L;

@@ -62,10 +62,62 @@ __device__ __forceinline__ void cm_load_site(const CmKP& p, int e, int n, int k,
   }
 }
 
+// Saturation adjustment (eq. 15): the root T of I*(T; rho, q_t) = I by Newton iterations with the analytical
+// derivative, I* from eq. (7)-(8) with the excess q_t - q_v*(T, rho) as liquid, q_v* = p*(T) / (rho R_v T) and the
+// closed-form p*(T) of a calorically perfect gas (Romps 2008).  Returns T; ql = liquid specific humidity.
+__device__ __forceinline__ double cm_sat_q(const CmThermo& th, double T, double rho) {
+  const double iT = 1.0 / T;
+  return th.p_tr * pow(T * th.iT_tr, th.sx1) * exp(th.sx2 * (th.iT_tr - iT)) * iT / (rho * th.R_v);
+}
+static __device__ __noinline__ double cm_sat_adjust(const CmThermo& th, double I, double rho, double qt, double& ql) {
+  double T = th.T_0 + (I - qt * th.I_v0) / (th.c_vd + th.b * qt);
+  if (qt <= cm_sat_q(th, T, rho)) { ql = 0.0; return T; }
+  for (int it = 0; it < 50; ++it) {
+    const double qs = cm_sat_q(th, T, rho), dT0 = T - th.T_0;
+    const double f = (1.0 - qt) * th.c_vd * dT0 + qs * (th.c_vv * dT0 + th.I_v0) + (qt - qs) * th.c_vl * dT0 - I;
+    const double dqs = qs * ((th.Lv0 + th.dcp * dT0) / (th.R_v * T * T) - 1.0 / T);
+    const double df = (1.0 - qt) * th.c_vd + qs * th.c_vv + (qt - qs) * th.c_vl + dqs * ((th.c_vv - th.c_vl) * dT0 + th.I_v0);
+    const double dT = f / df;
+    T -= dT;
+    if (fabs(dT) <= 1e-14 * T) break;
+  }
+  ql = qt - cm_sat_q(th, T, rho);
+  return T;
+}
+// pressure (eq. 13-14 with condensate), R_m and c_vm of moist air from (rho, I, q_t) under the saturation adjustment
+__device__ __forceinline__ double cm_sat_pressure(const CmThermo& th, double rho, double I, double qt, double& Rm, double& cvm) {
+  double ql;
+  const double T = cm_sat_adjust(th, I, rho, qt, ql);
+  Rm = th.R_d * (1.0 - qt) + th.R_v * (qt - ql);
+  cvm = th.c_vd * (1.0 - qt) + th.c_vv * (qt - ql) + th.c_vl * ql;
+  return rho * Rm * T;
+}
+
 // a1: primitive recovery (eq. 6-10, 13-14 with q_v = q_t) and p - p_r from state differences (R12)
-template <bool MOIST>
+// SAT: the kernel also carries the saturation-adjusted equation of state, chosen at run time by p.satadj
+template <bool MOIST, bool SAT = false>
 __device__ __forceinline__ void cm_eos(const CmKP& p, const double* Y, const CmSite& s, CmPrim& P) {
   const CmThermo& th = p.th;
+  if constexpr (MOIST && SAT) {
+    if (p.satadj) {
+      P.rho = Y[0]; P.ir = 1.0 / Y[0];
+      P.u = Y[1] * P.ir; P.v = Y[2] * P.ir; P.w = Y[3] * P.ir;
+      P.q = Y[5] * P.ir;
+      P.K = 0.5 * (Y[1] * P.u + Y[2] * P.v + Y[3] * P.w);
+      const double I = Y[4] * P.ir - 0.5 * (P.u * P.u + P.v * P.v + P.w * P.w) - s.Phi;
+      double Rm, cvm;
+      P.p = cm_sat_pressure(th, Y[0], I, P.q, Rm, cvm);
+      P.h = (Y[4] + P.p) * P.ir;
+      P.c2 = (1.0 + Rm / cvm) * P.p * P.ir;
+      if (p.use_ref) {
+        // p_r = pressure of the resting reference state under the same equation of state (no R12 with condensate)
+        double Rr, cr;
+        P.pp = P.p - cm_sat_pressure(th, s.rho_r, s.rhoe_r / s.rho_r - s.Phi, s.rhoq_r / s.rho_r, Rr, cr);
+        P.drho = Y[0] - s.rho_r;
+      } else { P.pp = P.p; P.drho = Y[0]; }
+      return;
+    }
+  }
   P.rho = Y[0];
   P.ir = cm_rcp(Y[0]);
   P.u = Y[1] * P.ir; P.v = Y[2] * P.ir; P.w = Y[3] * P.ir;
@@ -241,6 +293,49 @@ __device__ __forceinline__ void cm_surface_flux(const CmKP& p, const double* A, 
     const double c = sJ * rho * p.drag_cd * cm_sqrt(u0 * u0 + u1 * u1 + u2 * u2);
     r[1] -= c * u0; r[2] -= c * u1; r[3] -= c * u2;
   }
+}
+
+// Roe flux (Roe 1981): Fs = sJ n.F1* = (1/2)(A.F1^- + A.F1^+) - (1/2) sJ sum_k |lambda_k| alpha_k r_k with the
+// sqrt(rho)-weighted averages of u, h_tot and q.  With the mixture frozen at q~ the EOS is an ideal gas with
+// gamma - 1 = kappa~ and the energy shifted by s~ = Phi + q~ I_v0 - c_vm T_0, so c~^2 = kappa~ (H~ - s~ - |u~|^2 / 2);
+// rho q is a passive wave of speed u~_n.  Phi = geopotential of the face node.
+template <bool MOIST>
+__device__ __forceinline__ void cm_roe(const CmKP& p, const double* Ym, const CmPrim& Pm, const double* AFm, const double* Yp,
+                                       const CmPrim& Pp, const double* AFp, const double* A, double sJ, double Phi, double* Fs) {
+  constexpr int NV = MOIST ? 6 : 5;
+  const CmThermo& th = p.th;
+  const double isJ = 1.0 / sJ;
+  const double n[3] = {A[0] * isJ, A[1] * isJ, A[2] * isJ};
+  const double wm = sqrt(Ym[0]), wp = sqrt(Yp[0]), iw = 1.0 / (wm + wp);
+  const double um[3] = {Pm.u, Pm.v, Pm.w}, up[3] = {Pp.u, Pp.v, Pp.w};
+  double ut[3], du[3], un = 0.0, K = 0.0, dun = 0.0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    ut[i] = (wm * um[i] + wp * up[i]) * iw; du[i] = up[i] - um[i];
+    un += ut[i] * n[i]; K += 0.5 * ut[i] * ut[i]; dun += du[i] * n[i];
+  }
+  const double H = (wm * Pm.h + wp * Pp.h) * iw;
+  const double q = MOIST ? (wm * Pm.q + wp * Pp.q) * iw : 0.0;
+  const double cvm = th.c_vd + th.b * q, kappa = (th.R_d + th.a * q) / cvm;
+  const double sh = Phi + q * th.I_v0 - cvm * th.T_0;
+  const double c2 = kappa * (H - sh - K), cs = sqrt(c2);
+  const double rt = wm * wp;
+  const double drho = Yp[0] - Ym[0], dp = Pp.pp - Pm.pp;
+  const double a1 = (dp - rt * cs * dun) / (2.0 * c2), a5 = (dp + rt * cs * dun) / (2.0 * c2), a2 = drho - dp / c2;
+  const double l1 = fabs(un - cs), l2 = fabs(un), l5 = fabs(un + cs);
+  double D[6];
+  D[0] = l1 * a1 + l2 * a2 + l5 * a5;
+  double udu = 0.0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    const double shr = du[i] - dun * n[i];
+    D[1 + i] = l1 * a1 * (ut[i] - cs * n[i]) + l2 * (a2 * ut[i] + rt * shr) + l5 * a5 * (ut[i] + cs * n[i]);
+    udu += ut[i] * shr;
+  }
+  D[4] = l1 * a1 * (H - cs * un) + l2 * (a2 * (K + sh) + rt * udu) + l5 * a5 * (H + cs * un);
+  if (MOIST) D[5] = (l1 * a1 + l2 * a2 + l5 * a5) * q + l2 * rt * (Pp.q - Pm.q);
+#pragma unroll
+  for (int v = 0; v < NV; ++v) Fs[v] = 0.5 * (AFm[v] + AFp[v]) - 0.5 * sJ * D[v];
 }
 
 template <int NV>

@@ -108,6 +108,19 @@ def test_hllc_parity(P, oracle_mod, k):
     assert np.all(state_errors(g.to_host(Qd), o.lsrk54(Q, dt, 20)) <= STEP_TOL)
 
 
+@pytest.mark.parametrize("k", [1, 3, 4, 5])
+def test_roe_parity(P, oracle_mod, k):
+    cfg, Q, dt = small_config(k)
+    cfg = dict(cfg, riemann=2)
+    err = _rhs_check(P, oracle_mod, cfg, Q, dt)
+    assert np.all(err <= RHS_TOL), err
+    o = oracle_mod.Oracle(cfg); g = P.CmDg(cfg)
+    Qd = g.to_device(Q); g.lsrk_step(Qd, dt, 20)
+    assert np.all(state_errors(g.to_host(Qd), o.lsrk54(Q, dt, 20)) <= STEP_TOL)
+    with pytest.raises(P.CmDgError):
+        P.CmDg(dict(cfg, riemann=3))
+
+
 def test_curl_invariant_metrics_parity_and_free_stream(P, oracle_mod):
     from test_oracle_next import warped_3d
     cfg, Y = warped_3d(metric_form=1, sgs=1)
