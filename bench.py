@@ -276,6 +276,31 @@ def bench_leg(P, torch, cfg, Q, dt, steps, peak, label, bytes_per_node_stage):
     return out
 
 
+LEGS = {
+    "c3": (lambda W: W.config3(), 20, "config 3 (dry CBL, SL, flat) 32x32x16", (5, 1, False)),
+    "c3x": (lambda W: W.config3(ne=(96, 96, 48), hi=(19200.0, 19200.0, 9000.0)), 5, "config 3 scaled to 96x96x48 elements", (5, 1, False)),
+    "c4": (lambda W: W.config4(), 20, "config 4 (mountain, inviscid, stored metrics) 120x1x30", (5, 0, True)),
+    "c4x": (lambda W: W.config4(ne=(120, 96, 30)), 5, "config 4 extruded to 120x96x30 elements", (5, 0, True)),
+}
+
+
+def one_leg(P, torch, name, peak):
+    """One of the further workloads by name (also `bench.py --leg NAME`, the command the ncu captures of the stored-metric
+    kernels run).  For the stored-metric legs the bytes those kernels really move are reported beside the algorithmic
+    ones: they read 12 geometry fields (Ja 9, 1/J, z, tau_s) and 2 reference fields per node that the 2.5-D-specialised
+    count of SURVEY 8(d) replaces by 5 values."""
+    import workloads as W
+    make, steps, label, sb = LEGS[name]
+    cfg, Q, dt = make(W)
+    out = bench_leg(P, torch, cfg, Q, dt, steps, peak, label, stage_bytes(*sb))
+    if sb[2]:
+        moved = (5 + 5 + 5 + 5 - 1.0) * 8 + (12 + 2) * 8          # Q, residual (4 of 5 stages), residual out, Q out + geometry + reference
+        out["moved_bytes_per_node_stage"] = moved
+        out["moved_gbs"] = out["achieved_gbs"] * moved / out["algorithmic_bytes_per_node_stage"]
+        out["moved_frac_of_measured_hbm"] = out["moved_gbs"] / peak
+    return out
+
+
 def extra_legs(P, torch, args, peak):
     """Order sweep of config 5 at ~55 M nodes (N = 3, 5, 6), dry config 3 and terrain config 4 (BASELINE size and a
     y-extruded variant that fills the GPU): throughput and whole-stage roofline fraction of each."""
@@ -288,14 +313,8 @@ def extra_legs(P, torch, args, peak):
         cfg, Q, dt = W.config5(ne=ne, N=N, hi=(6000.0, 6000.0, 3000.0))
         out["sweep"].append(bench_leg(P, torch, cfg, Q, dt, 3, peak, "config 5 at N=%d, %dx%dx%d" % ((N,) + tuple(ne)), stage_bytes(6, 1, False)))
         del cfg, Q
-    cfg, Q, dt = W.config3()
-    out["configs"].append(bench_leg(P, torch, cfg, Q, dt, 20, peak, "config 3 (dry CBL, SL, flat) 32x32x16", stage_bytes(5, 1, False)))
-    cfg, Q, dt = W.config3(ne=(96, 96, 48), hi=(19200.0, 19200.0, 9000.0))
-    out["configs"].append(bench_leg(P, torch, cfg, Q, dt, 5, peak, "config 3 scaled to 96x96x48 elements", stage_bytes(5, 1, False)))
-    cfg, Q, dt = W.config4()
-    out["configs"].append(bench_leg(P, torch, cfg, Q, dt, 20, peak, "config 4 (mountain, inviscid, stored metrics) 120x1x30", stage_bytes(5, 0, True)))
-    cfg, Q, dt = W.config4(ne=(120, 96, 30))
-    out["configs"].append(bench_leg(P, torch, cfg, Q, dt, 5, peak, "config 4 extruded to 120x96x30 elements", stage_bytes(5, 0, True)))
+    for name in ("c3", "c3x", "c4", "c4x"):
+        out["configs"].append(one_leg(P, torch, name, peak))
     return out
 
 
@@ -464,6 +483,7 @@ def main():
     ap.add_argument("--record-traffic", default=None, metavar="RAW.csv",
                     help="store the tendency kernel's ncu DRAM bytes (ncu --page raw --csv export) in profiles/traffic.json")
     ap.add_argument("--no-extra", action="store_true", help="skip the extra legs (order sweep, configs 3 and 4)")
+    ap.add_argument("--leg", default=None, choices=sorted(LEGS), help="run ONE of the further workloads and print its report")
     ap.add_argument("--tuning", nargs="*", default=None, metavar="KEY=VAL",
                     help="cm_dg_tuning fields for kernel experiments (e.g. kernel=7 row_len=16); default: the library's defaults")
     args = ap.parse_args()
@@ -476,6 +496,10 @@ def main():
         args.ne = list(W.SWEEP5[args.order])
     if args.record_traffic:
         record_traffic(args)
+    elif args.leg:
+        import torch
+        import paper_2110_00853_b200 as P
+        print(json.dumps(one_leg(P, torch, args.leg, measured_peaks()[0])))
     elif args.impl == "reference":
         run_reference(args)
     else:

@@ -99,7 +99,8 @@ typedef struct {
   int32_t max_chunk;     /* tiled order: longest x-chunk L (L divides Ex), 0 = 32                                       */
   int32_t max_patch;     /* tiled order: tallest y-patch PY (PY divides Ey), 0 = 16                                     */
   int32_t force_general; /* 1: use the stored-metric kernels (the path of warped meshes) on a flat mesh too             */
-  int32_t kernel;        /* 0 default | 10 row-sweep kernels (flat) | 7 CTA-per-element kernels (flat) | 2 stored-metric */
+  int32_t kernel;        /* 0 default | 10 row-sweep kernels (flat) | 7 CTA-per-element kernels (flat) | 11 CTA-per-element
+                            tendency kernel of stored-metric meshes (their default) | 2 thread-per-node stored-metric kernels */
   int32_t ahead_t;       /* kernel 7: L2 prefetch distance of the tendency kernel in elements; -1 one wave, 0 off       */
   int32_t ahead_g;       /* same for the gradient kernel                                                                */
   int32_t row_len;       /* kernel 10: elements per row sweep (must divide the x-chunk), 0 = the whole chunk            */

@@ -535,7 +535,7 @@ void numerical_flux(const Ctx& c, const double* Ym, const Prim& Pm, const double
     // sqrt(rho)-weighted averages u~, H~ (total enthalpy), q~.  With the mixture frozen at q~ the EOS of eq. (6)-(14) is an
     // ideal gas with gamma - 1 = kappa~ = R_m / c_vm and the energy shifted by s~ = Phi + q~ I_v0 - c_vm T_0:
     // p = kappa (rho e - rho |u|^2 / 2 - rho s), hence c~^2 = kappa~ (H~ - s~ - |u~|^2 / 2).  Exact Roe linearisation for dry
-    // air; rho q is a passive wave of speed u~_n (reading R30).  No entropy fix.
+    // air; rho q is a passive wave of speed u~_n (reading R32).  No entropy fix.
     double wm = std::sqrt(Ym[0]), wp = std::sqrt(Yp[0]), iw = 1.0 / (wm + wp);
     double ut[3], un = 0, K = 0;
     for (int i = 0; i < 3; ++i) { ut[i] = (wm * Pm.u[i] + wp * Pp.u[i]) * iw; un += ut[i] * nrm[i]; K += 0.5 * ut[i] * ut[i]; }

@@ -42,6 +42,9 @@ def build(force=False, verbose=False):
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     extra = os.environ.get("CM_DG_NVCC_EXTRA", "").split()
     LIB = os.environ.get("CM_DG_LIB_OUT", globals()["LIB"])
+    if extra and LIB == globals()["LIB"]:
+        raise RuntimeError("CM_DG_NVCC_EXTRA builds an experimental variant: set CM_DG_LIB_OUT to a path other than the "
+                           "default library, which tests and bench load")
     if not force and not extra and not _stale(LIB):
         return LIB
     os.makedirs(OBJ, exist_ok=True)

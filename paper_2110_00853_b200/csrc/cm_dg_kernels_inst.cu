@@ -4,6 +4,7 @@
 #include "cm_dg_kernels2.cuh"
 #include "cm_dg_kernels7.cuh"
 #include "cm_dg_kernels10.cuh"
+#include "cm_dg_kernels11.cuh"
 
 #ifndef CM_NQ
 #error "compile with -DCM_NQ=<N+1>"
@@ -164,6 +165,27 @@ cudaError_t launch_tend10m(const CmKP& kp, cudaStream_t st) {
   return (kp.rka != 0.0) ? launch_tend10<Nq, MOIST, SGS, 1>(kp, st) : launch_tend10<Nq, MOIST, SGS, 2>(kp, st);
 }
 
+// CTA-per-element tendency kernel of stored-metric meshes (cm_dg_kernels11.cuh): grid = the tiled element order
+template <int Nq, bool MOIST, bool SGS, int MODE>
+cudaError_t launch_tend11(const CmKP& kp, cudaStream_t st) {
+  using C = CmCfg7<Nq, MOIST>;
+  using R = CmCfg11<Nq, MOIST, SGS, MODE>;
+  static LaunchState ls;
+  int wave = 0;
+  cudaError_t err = configure(cm11_tendency_kernel<Nq, MOIST, SGS, MODE>, R::SMEM, ls, C::THREADS, &wave);
+  if (err != cudaSuccess) return err;
+  CmKP k2 = kp;
+  if (k2.ahead < 0) k2.ahead = wave;
+  cm11_tendency_kernel<Nq, MOIST, SGS, MODE><<<dim3(kp.gPY * kp.gL, kp.gEz, kp.gNXC * kp.gNYP), C::THREADS, R::SMEM, st>>>(k2);
+  return cudaGetLastError();
+}
+
+template <int Nq, bool MOIST, bool SGS>
+cudaError_t launch_tend11m(const CmKP& kp, cudaStream_t st) {
+  if (kp.mode == 0) return launch_tend11<Nq, MOIST, SGS, 0>(kp, st);
+  return (kp.rka != 0.0) ? launch_tend11<Nq, MOIST, SGS, 1>(kp, st) : launch_tend11<Nq, MOIST, SGS, 2>(kp, st);
+}
+
 }  // namespace
 
 cudaError_t CM_CAT(cm_launch_gradient_nq, CM_NQ)(const CmKP& kp, int moist, int general, int variant, cudaStream_t st) {
@@ -189,6 +211,12 @@ cudaError_t CM_CAT(cm_launch_tendency_nq, CM_NQ)(const CmKP& kp, int moist, int 
   if (variant == 7 && !general) {
     if (kp.sgs) return moist ? launch_tend7m<CM_NQ, true, true>(kp, st) : launch_tend7m<CM_NQ, false, true>(kp, st);
     return moist ? launch_tend7m<CM_NQ, true, false>(kp, st) : launch_tend7m<CM_NQ, false, false>(kp, st);
+  }
+  if constexpr (CmCfg11<CM_NQ, true, true, 1>::OK) {   // one predicate per order
+    if (variant == 11 && general) {
+      if (kp.sgs) return moist ? launch_tend11m<CM_NQ, true, true>(kp, st) : launch_tend11m<CM_NQ, false, true>(kp, st);
+      return moist ? launch_tend11m<CM_NQ, true, false>(kp, st) : launch_tend11m<CM_NQ, false, false>(kp, st);
+    }
   }
   if (moist) return general ? launch_tend2<CM_NQ, true, 1>(kp, st) : launch_tend2<CM_NQ, true, 0>(kp, st);
   return general ? launch_tend2<CM_NQ, false, 1>(kp, st) : launch_tend2<CM_NQ, false, 0>(kp, st);

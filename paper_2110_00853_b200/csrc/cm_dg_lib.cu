@@ -501,6 +501,7 @@ struct cm_dg_ctx {
   cm_dg_params prm;
   int N, Nq, Np, nvar, ngrad, general, moist;
   int variant = 10;  // 10: row-sweep kernels (cm_dg_kernels10.cuh; flat bricks); 7: CTA-per-element kernels (cm_dg_kernels7.cuh; flat bricks);
+                     // 11: CTA-per-element tendency kernel for stored-metric meshes (cm_dg_kernels11.cuh) + thread-per-node gradient;
                      // 2: thread-per-node kernels (cm_dg_kernels2.cuh; any geometry); cm_dg_tuning::kernel selects
   int64_t Ne, stride;
   cudaStream_t st;
@@ -618,7 +619,7 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   std::memset(&tn, 0, sizeof(tn));
   tn.ahead_t = tn.ahead_g = -1;
   if (tune) tn = *tune;
-  if (tn.kernel != 0 && tn.kernel != 2 && tn.kernel != 7 && tn.kernel != 10) return fail(CM_DG_EINVAL, "cm_dg_setup_tuned: kernel must be 0, 2, 7 or 10");
+  if (tn.kernel != 0 && tn.kernel != 2 && tn.kernel != 7 && tn.kernel != 10 && tn.kernel != 11) return fail(CM_DG_EINVAL, "cm_dg_setup_tuned: kernel must be 0, 2, 7, 10 or 11");
   if (tn.max_chunk < 0 || tn.max_patch < 0 || tn.row_len < 0) return fail(CM_DG_EINVAL, "cm_dg_setup_tuned: negative tile size");
   *out = nullptr;
   if (p->N < 2 || p->N > 7) return fail(CM_DG_EINVAL, "cm_dg_setup: polynomial order N must be in 2..7");
@@ -736,10 +737,12 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   c->general = (p->geom != 0 || (p->use_ref && !ref_z_only) || p->metric_form == 1) ? 1 : 0;
   if (tn.force_general) c->general = 1;
   if (tn.kernel) c->variant = tn.kernel;
-  if (c->general) c->variant = 2;
-  // HLLC is implemented in the thread-per-node kernels; so is the Richardson factor at the orders whose flat gradient
-  // kernel is the trace-buffer one (N <= 3)
-  if (p->riemann != 0 || p->satadj || (p->richardson && Nq <= 4)) c->variant = 2;
+  // stored-metric meshes: CTA-per-element tendency kernel fed by bulk TMA (cm_dg_kernels11.cuh) with the thread-per-node
+  // gradient kernel; kernel = 2 keeps the thread-per-node tendency kernel as well
+  if (c->general) c->variant = (tn.kernel == 2) ? 2 : 11;
+  // HLLC, Roe and the saturation adjustment are implemented in the thread-per-node kernels; so is the Richardson factor at
+  // the orders whose flat gradient kernel is the trace-buffer one (N <= 3)
+  if (p->riemann != 0 || p->satadj || (!c->general && p->richardson && Nq <= 4)) c->variant = 2;
 
   auto bail = [&](int code) { free_ctx(c); return code; };
 #define CM_CUDA_B(call)                                                                                   \
@@ -786,6 +789,7 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
     if (L % tn.row_len != 0) { fail(CM_DG_EINVAL, "cm_dg_setup_tuned: row_len must divide the x-chunk length"); return bail(CM_DG_EINVAL); }
     kp.gS = tn.row_len;
   }
+  if (c->variant == 11 && (p->ne[2] > 65535 || (int64_t)kp.gNXC * kp.gNYP > 65535)) c->variant = 2;   // 1-D grid instead
   if (c->variant != 2 && ((int64_t)PY * L > 2147483647LL || p->ne[2] > 65535 || (int64_t)kp.gNXC * kp.gNYP > 65535)) {   // 3-D grid of the flat kernels
     fail(CM_DG_EINVAL, "cm_dg_setup: mesh exceeds the launch-grid limits (Ez and (Ex/L)*(Ey/PY) must be <= 65535)");
     return bail(CM_DG_EINVAL);

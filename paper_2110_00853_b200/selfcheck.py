@@ -9,7 +9,7 @@ summation order, so any difference is an ordering bug in the mbarrier / cp.async
 
 One cm_dg_rhs and two cm_dg_lsrk_step calls per case on small seeded meshes: the row-sweep, CTA-per-element and
 stored-metric kernels, both L2-prefetch settings, walls and periodic sides, dry and moist, every closure, the sponge,
-the element filter, HLLC and the curl-invariant metrics.  Prints one line per case; exits non-zero on a non-finite result.
+the element filter, HLLC / Roe, surface fluxes, the saturation adjustment and the horizontal statistics.  Prints one line per case; exits non-zero on a non-finite result.
 """
 import sys
 
@@ -35,7 +35,11 @@ def main():
         ("config4 terrain", c4(), None), ("config4 terrain + closure", c4(sgs=1), None),
         ("config5 Vreman + Richardson", c5(sgs=2, richardson=1), None),
         ("config4 sponge + filter", c4(sponge_alpha=0.4, sponge_zs=2500.0, u_relax=(10.0, 0.0, 0.0), filter_order=64), None),
-        ("config5 filter", c5(filter_order=64), None), ("config3 HLLC", c3(riemann=1), None),
+        ("config5 filter", c5(filter_order=64), None), ("config3 HLLC", c3(riemann=1), None), ("config3 Roe", c3(riemann=2), None),
+        ("config5 surface fluxes", c5(drag_cd=1.3e-3, lhf_bottom=147.2, evap_bottom=5.9e-5), None),
+        ("config5 surface fluxes cm7", c5(drag_cd=1.3e-3, lhf_bottom=147.2, evap_bottom=5.9e-5), {"kernel": 7}),
+        ("config5 saturation adjustment", c5(satadj=1), None),
+        ("config5 long rows", (W.config5(ne=(32, 4, 3), N=4, hi=(2000.0, 250.0, 187.5)), {}), None),
     ]
     bad = 0
     for name, ((cfg, Q, dt), over), tuning in cases:
@@ -48,8 +52,10 @@ def main():
             g.lsrk_step(Qd, dt, 2)
             runs.append((dQ, Qd))
         d = g.diagnostics(runs[0][1])
+        prof = [g.profiles(runs[0][1]) for _ in range(2)]
+        same_prof = bool(np.array_equal(prof[0], prof[1]))
         finite = bool(torch.isfinite(runs[0][0]).all()) and d["n_nonfinite"] == 0
-        same = all(bool((r[0] == runs[0][0]).all()) and bool((r[1] == runs[0][1]).all()) for r in runs[1:])
+        same = same_prof and all(bool((r[0] == runs[0][0]).all()) and bool((r[1] == runs[0][1]).all()) for r in runs[1:])
         bad += 0 if (finite and same) else 1
         print("%-32s %s %s  mass %.12e" % (name, "finite" if finite else "NON-FINITE", "bitwise-repeatable" if same else "NOT REPEATABLE", d["mass"]))
         g.close()
