@@ -103,7 +103,8 @@ typedef struct {
                             tendency kernel of stored-metric meshes (their default) | 2 thread-per-node stored-metric kernels */
   int32_t ahead_t;       /* kernel 7: L2 prefetch distance of the tendency kernel in elements; -1 one wave, 0 off       */
   int32_t ahead_g;       /* same for the gradient kernel                                                                */
-  int32_t row_len;       /* kernel 10: elements per row sweep (must divide the x-chunk), 0 = the whole chunk            */
+  int32_t row_len;       /* kernel 10: elements per row sweep (must divide the x-chunk), 0 = chosen by the library: the
+                            whole chunk on large meshes, shorter rows (>= 8) where that leaves fewer than 4 waves of CTAs   */
 } cm_dg_tuning;
 
 /* Conservation integrals and step-size ingredients (eq. 57; eq. 61-62). */

@@ -117,7 +117,8 @@ template <int Nq, bool MOIST> struct CmCfg7 {
 #ifndef CM_G_REGTHREADS
 #define CM_G_REGTHREADS 896
 #endif
-  static constexpr int MINB_T = cap(fit(TEND_SMEM), cap(CM_T_REGTHREADS / THREADS, 16));   // 640: >= 100 registers per thread
+  // 640: >= 100 registers per thread; the largest CTA that still fits twice (N = 6: 352 threads) is held to 93 registers
+  static constexpr int MINB_T = cap(fit(TEND_SMEM), cap((THREADS > 320 && THREADS <= 352 ? 704 : CM_T_REGTHREADS) / THREADS, 16));
   static constexpr int MINB_G = cap(fit(GRAD_SMEM), cap(896 / THREADS, 16));   // >= 72 registers per thread
 };
 

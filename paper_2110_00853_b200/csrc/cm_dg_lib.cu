@@ -784,7 +784,19 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   for (int d = 0; d < 3; ++d) kp.gbc[d] = p->bc[d];
   kp.ahead = -1;   // L2 prefetch distance of the cm7 kernels: -1 = one wave of resident CTAs (set by the launcher)
   c->ahead_t = tn.ahead_t; c->ahead_g = tn.ahead_g;
-  kp.gS = L;       // row-sweep kernels: a row is a whole x-chunk unless the tuning asks for shorter rows
+  kp.gS = L;       // row-sweep kernels: a row is a whole x-chunk unless the mesh is small or the tuning asks for shorter rows
+  {
+    // small meshes: long rows leave too few CTAs for an even last wave (config 3 at 32x32x16: 512 rows of 32 on 444 CTA
+    // slots, 7.1 G DOF-stages/s; rows of 8: 8.6 G).  Longest row that still gives >= 4 waves of 3 CTAs per SM, but not
+    // below 8 elements (the pipeline fill of a row is one element)
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    const int64_t want = (int64_t)4 * 3 * sms;
+    int best = 0;
+    for (int S = L; S >= 1; --S) if (L % S == 0 && Ne / S >= want) { best = S; break; }
+    if (best < 8) { best = L; for (int S = 8; S <= L; ++S) if (L % S == 0) { best = S; break; } }
+    kp.gS = best;
+  }
   if (tn.row_len > 0) {
     if (L % tn.row_len != 0) { fail(CM_DG_EINVAL, "cm_dg_setup_tuned: row_len must divide the x-chunk length"); return bail(CM_DG_EINVAL); }
     kp.gS = tn.row_len;
