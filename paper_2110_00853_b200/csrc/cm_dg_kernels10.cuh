@@ -18,8 +18,9 @@
 //     the residual is staged at the top of the iteration that consumes it;
 //   * every asynchronous copy (bulk TMA and the cp.async gathers) is issued by a dedicated PRODUCER warp, so that the
 //     ~20 issue cycles per bulk copy and the address arithmetic of the gathers never sit on the critical path of the
-//     compute warps; the compute warps synchronise among themselves with a named barrier, with the producer once per
-//     element (buffers free), and with the data through mbarriers.
+//     compute warps; the compute warps synchronise among themselves with a named barrier (twice per element), hand the
+//     buffers of a finished element back to the producer with a non-blocking bar.arrive (only the producer waits), and
+//     wait for data on mbarriers.
 // The element-level phases (1: EOS + contravariant fluxes, 2: line tasks + face tasks, 3: assembly + fused LSRK update)
 // and their arithmetic are those of cm_dg_kernels7.cuh; this file reuses its device functions.  P:L<n> = paper line.
 #pragma once

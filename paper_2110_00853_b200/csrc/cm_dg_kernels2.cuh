@@ -1,6 +1,6 @@
 // cm_dg_kernels2.cuh -- thread-per-node kernels for ANY geometry (stored metric terms, per-node reference state): the
-// path of warped meshes (geom != 0) and of reference states that are not columns; on flat bricks the CTA-per-element
-// kernels of cm_dg_kernels7.cuh are used instead (CM_DG_KERNEL=2 forces these).
+// path of warped meshes (geom != 0) and of reference states that are not columns; on flat bricks the row-sweep /
+// CTA-per-element kernels are used instead (cm_dg_tuning.kernel = 2 forces these).
 //   * one thread owns ONE node, a CTA holds EPB elements x TPE threads (~64-100 registers per thread, several CTAs per
 //     SM): latency is hidden by thread-level parallelism;
 //   * the tensor-product contractions are done by LINE tasks: a thread owns one xi/eta/zeta line of one element,
@@ -9,7 +9,10 @@
 //   * face work is a list of 6*Nq^2 FACE tasks per element spread evenly over the CTA's threads; a face whose
 //     neighbour element lives in the same CTA reads the neighbour's state and contravariant flux straight from
 //     shared memory (no global loads, no second EOS / flux evaluation); only CTA-external faces go to L2.
-// Parity-tested on all five configs; not tuned (profiles/r1a_v2.md is its only capture).  P:L<n> = paper line.
+// On stored-metric meshes the tendency kernel of cm_dg_kernels11.cuh (CTA per element, bulk-TMA staging) is the default
+// and this file serves the gradient, the HLLC / Roe fluxes and the saturation-adjusted equation of state; kernel = 2 selects
+// the tendency kernel below as well.  Both kernels prefetch the arrays of the element one wave of CTAs ahead into L2.
+// Parity-tested on all five configs; profile: profiles/r2_stored_metric.md.  P:L<n> = paper line.
 #pragma once
 #include "cm_dg_internal.h"
 #include "cm_dg_physics.cuh"
