@@ -281,6 +281,7 @@ LEGS = {
     "c3x": (lambda W: W.config3(ne=(96, 96, 48), hi=(19200.0, 19200.0, 9000.0)), 5, "config 3 scaled to 96x96x48 elements", (5, 1, False)),
     "c4": (lambda W: W.config4(), 20, "config 4 (mountain, inviscid, stored metrics) 120x1x30", (5, 0, True)),
     "c4x": (lambda W: W.config4(ne=(120, 96, 30)), 5, "config 4 extruded to 120x96x30 elements", (5, 0, True)),
+    "c4s": (lambda W: W.config4(ne=(120, 96, 30), sgs=1), 5, "config 4 extruded to 120x96x30 elements, with the Smagorinsky-Lilly closure", (5, 1, True)),
 }
 
 
@@ -295,6 +296,8 @@ def one_leg(P, torch, name, peak):
     out = bench_leg(P, torch, cfg, Q, dt, steps, peak, label, stage_bytes(*sb))
     if sb[2]:
         moved = (5 + 5 + 5 + 5 - 1.0) * 8 + (12 + 2) * 8          # Q, residual (4 of 5 stages), residual out, Q out + geometry + reference
+        if sb[1]:
+            moved += (5 + 15 + 9) * 8 + 9 * 8                     # gradient sweep: Q, 15 geometry fields, G out; G read by the tendency
         out["moved_bytes_per_node_stage"] = moved
         out["moved_gbs"] = out["achieved_gbs"] * moved / out["algorithmic_bytes_per_node_stage"]
         out["moved_frac_of_measured_hbm"] = out["moved_gbs"] / peak
@@ -313,7 +316,7 @@ def extra_legs(P, torch, args, peak):
         cfg, Q, dt = W.config5(ne=ne, N=N, hi=(6000.0, 6000.0, 3000.0))
         out["sweep"].append(bench_leg(P, torch, cfg, Q, dt, 3, peak, "config 5 at N=%d, %dx%dx%d" % ((N,) + tuple(ne)), stage_bytes(6, 1, False)))
         del cfg, Q
-    for name in ("c3", "c3x", "c4", "c4x"):
+    for name in ("c3", "c3x", "c4", "c4x", "c4s"):
         out["configs"].append(one_leg(P, torch, name, peak))
     return out
 

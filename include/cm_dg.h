@@ -105,6 +105,8 @@ typedef struct {
   int32_t ahead_g;       /* same for the gradient kernel                                                                */
   int32_t row_len;       /* kernel 10: elements per row sweep (must divide the x-chunk), 0 = chosen by the library: the
                             whole chunk on large meshes, shorter rows (>= 8) where that leaves fewer than 4 waves of CTAs   */
+  int32_t no_graph;      /* 1: cm_dg_lsrk_step* always launch kernel by kernel; 0: a time step is captured as a CUDA graph on
+                            the second consecutive call with the same (Q_dev, dt, table) and replayed afterwards           */
 } cm_dg_tuning;
 
 /* Conservation integrals and step-size ingredients (eq. 57; eq. 61-62). */
@@ -155,7 +157,7 @@ int cm_dg_gradient(cm_dg_ctx* ctx, const double* Q_dev, double* G_dev);
 int cm_dg_rhs(cm_dg_ctx* ctx, const double* Q_dev, double* dQ_dev, double t);
 
 /* a1-a5: advance Q by nsteps LSRK54 steps of size dt; every stage is one gradient kernel plus one fused
- * tendency + low-storage update kernel.  The result is left in Q_dev: the five stages of a step cycle through two
+ * tendency + low-storage update kernel (replayed from a CUDA graph of one step once the same Q_dev, dt have been seen twice).  The result is left in Q_dev: the five stages of a step cycle through two
  * ctx-owned buffers and end in the caller's array (no stage updates in place, no copy is appended). */
 int cm_dg_lsrk_step(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t nsteps);
 

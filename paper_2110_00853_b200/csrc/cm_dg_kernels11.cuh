@@ -1,6 +1,6 @@
-// cm_dg_kernels11.cuh -- CTA-per-element tendency kernel for STORED-METRIC meshes (geom != 0: terrain-following and fully
-// warped bricks, per-node reference state): the decomposition of cm7_tendency_kernel (cm_dg_kernels7.cuh) with the
-// geometry as data.
+// cm_dg_kernels11.cuh -- CTA-per-element tendency and gradient kernels for STORED-METRIC meshes (geom != 0: terrain-
+// following and fully warped bricks, per-node reference state): the decomposition of the flat CTA-per-element kernels
+// (cm_dg_kernels7.cuh) with the geometry as data.
 //
 // Why (profiles/r2_stored_metric.md): the thread-per-node kernel of cm_dg_kernels2.cuh waits on global loads at the start of
 // every phase (ncu: 38 % of its warp time in long-scoreboard stalls, 20 % at barriers, 0.43 eligible warps per scheduler).
@@ -293,6 +293,210 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg11<Nq, MOIST,
         o2 += p.stride;
       }
       o1 += p.stride;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2 on stored-metric meshes: BR1 auxiliary gradient + eddy-viscosity closure, same staging as the tendency kernel above.
+//   own tiles by bulk TMA: Q (NV) and the geometry fields 0..14 (Ja 9, 1/J, z, (C_s Delta)^2, Delta_m^2 3);
+//   neighbour traces by cp.async: Q (NV) and z of the neighbour's node;
+//   phase 1: gradient variables s = u, v, w, h_tot, [q_t], [theta_v] in place of the state (eq. 33, 35, 37, 40);
+//   phase 2: face tasks  s* - s^- = (s^+ - s^-)/2 (eq. 30-31), wall: u* = u - (n.u) n with n from Ja^d (A6), scalars kept (A8);
+//            line tasks  D_d s in reference space;
+//   phase 3: lifted jumps, G = (1/J) sum_d Ja^d (D_d s + lift_d) (eq. 28-29 with eq. 24), closure, field-major store.
+// RAW: the 15 raw gradients (cm_dg_gradient) | packed SGS fluxes (hot path).  RICH: theta_v is a further variable (eq. 40).
+// ------------------------------------------------------------------------------------------------
+template <int Nq, bool MOIST, bool RICH> struct CmCfg11G {
+  using C = CmCfg7<Nq, MOIST>;
+  static constexpr int NF = C::NF, NP = C::NP, NV = C::NV, SLOT = C::SLOT, THREADS = C::THREADS;
+  static constexpr int NS0 = C::NS;                     // u, v, w, h_tot, [q_t]
+  static constexpr int NS = NS0 + (RICH ? 1 : 0);       // + theta_v (<= NV: the variables replace the state in place)
+  static constexpr int NGEO = 15;                       // CmKP::geo fields 0..14
+  static constexpr int NTR = NV + 1;                    // trace values per face node: state, z
+  static constexpr int TS = C::fstride(NTR);
+  static constexpr int OFF_Q = 0;                                        // [NV][SLOT]
+  static constexpr int OFF_D = OFF_Q + NV * SLOT;                        // [3][NS][SLOT]
+  static constexpr int OFF_GEO = OFF_D + 3 * NS * SLOT;                  // [NGEO][SLOT]
+  static constexpr int OFF_T = OFF_GEO + NGEO * SLOT;                    // [6][TS]
+  static constexpr int OFF_M = OFF_T + 5 * TS + NTR * NF + (NTR * NF & 1);
+  static constexpr int DOUBLES = OFF_M + 2;
+  static constexpr size_t SMEM = sizeof(double) * DOUBLES;
+  static constexpr bool OK = SMEM <= 115712;
+  static constexpr int MINB = C::cap(C::fit(SMEM), C::cap(896 / THREADS, 16));
+  static_assert(NS <= NV, "gradient variables are stored in the state tiles");
+};
+
+template <int Nq, int NS, int SLOT, int D>
+__device__ __forceinline__ void cm11_grad_line(const CmKP& p, const double* __restrict__ ss, double* __restrict__ dd, int l) {
+  constexpr int NF = Nq * Nq, STR = Cm7Str<Nq, D>::value;
+  const int b = l / Nq, a = l - b * Nq;
+  const int base = (D == 0) ? Nq * l : (D == 1) ? a + NF * b : l;
+#pragma unroll
+  for (int v = 0; v < NS; ++v) {
+    const double* in = ss + v * SLOT + base;
+    double* out = dd + v * SLOT + base;
+    double x[Nq];
+#pragma unroll
+    for (int m = 0; m < Nq; ++m) x[m] = in[m * STR];
+#pragma unroll
+    for (int i = 0; i < Nq; ++i) {
+      double s = 0.0;
+#pragma unroll
+      for (int m = 0; m < Nq; ++m) s += p.D[i][m] * x[m];
+      out[i * STR] = s;
+    }
+  }
+}
+
+template <int Nq, bool MOIST, bool RAW, bool RICH>
+__global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg11G<Nq, MOIST, RICH>::MINB) cm11_gradient_kernel(const __grid_constant__ CmKP p) {
+  using C = CmCfg7<Nq, MOIST>;
+  using R = CmCfg11G<Nq, MOIST, RICH>;
+  constexpr int NF = C::NF, NP = C::NP, N = Nq - 1, NV = C::NV, SLOT = C::SLOT, NFP = C::NFP, THREADS = C::THREADS;
+  constexpr int NS0 = R::NS0, NS = R::NS, TS = R::TS, NGEO = R::NGEO;
+  extern __shared__ __align__(128) double smem11[];
+  double* Qt = smem11 + R::OFF_Q;
+  double* dt_ = smem11 + R::OFF_D;
+  double* Gt = smem11 + R::OFF_GEO;
+  double* T = smem11 + R::OFF_T;
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(smem11 + R::OFF_M);
+
+  const int t = threadIdx.x;
+  const Cm7Pos pos = cm7_position(p);
+  const int e = pos.e;
+  const int sh = C::ODD ? (e & 1) : 0;
+  if (t == THREADS - 32) { cm7_mbar_init(mbar, 1); cm7_fence_mbar_init(); }
+  __syncthreads();
+  if (t == THREADS - 32) {
+    const long long src = (long long)e * NP - sh;
+    const uint32_t mb = cm7_saddr(mbar);
+    cm7_mbar_expect_tx(mbar, (uint32_t)((NV + NGEO) * SLOT * sizeof(double)));
+    uint32_t d = cm7_saddr(Qt);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) { cm7_bulk_g2s_raw(d, p.Q + (size_t)v * p.stride + src, SLOT * 8, mb); d += SLOT * 8; }
+    d = cm7_saddr(Gt);
+#pragma unroll
+    for (int k = 0; k < NGEO; ++k) { cm7_bulk_g2s_raw(d, p.geo + (size_t)k * p.stride + src, SLOT * 8, mb); d += SLOT * 8; }
+  } else if (t > THREADS - 32 && p.ahead > 0 && e + p.ahead < p.Ne) {
+    const int ea = e + p.ahead;
+    const long long src = (long long)ea * NP - (C::ODD ? (ea & 1) : 0);
+    for (int j = t - (THREADS - 32) - 1; j < NV + NGEO; j += 31)
+      cm7_prefetch_l2((j < NV ? p.Q + (size_t)j * p.stride : p.geo + (size_t)(j - NV) * p.stride) + src, SLOT * 8);
+  }
+  for (int fn = THREADS - 1 - t; fn < 6 * NF; fn += THREADS) {   // neighbour traces: the thread that runs the face task copies them
+    int f, m, d, s, nm, np_, kline;
+    cm7_face_node<Nq>(fn, f, m, d, s, nm, np_, kline);
+    if (!((pos.wallmask >> f) & 1)) {
+      const size_t idp = (size_t)cm7_neighbour(p, pos, d, s) * NP + np_;
+      double* dst = T + f * TS + m;
+      const double* src = p.Q + idp;
+#pragma unroll
+      for (int v = 0; v < NV; ++v) { cm7_cp8(dst + v * NF, src); src += p.stride; }
+      cm7_cp8(dst + NV * NF, p.geo + 10 * p.stride + idp);
+    }
+  }
+  cm7_cp_commit();
+
+  double* ss = Qt + sh; double* dd = dt_ + sh; const double* geo = Gt + sh;
+  const int n = t;
+  const bool node = t < NP;
+  const int k_ = n / NF, j_ = (n - k_ * NF) / Nq, i_ = n - k_ * NF - j_ * Nq;
+  cm7_mbar_wait(mbar, 0);
+
+  // ---- phase 1: gradient variables of the own node, in place of the state
+  if (node) {
+    double Y[6], s[6];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) Y[v] = ss[v * SLOT + n];
+    cm7_eos_grad<MOIST, RICH>(p, Y, p.th.grav * geo[10 * SLOT + n], s);
+#pragma unroll
+    for (int v = 0; v < NS; ++v) ss[v * SLOT + n] = s[v];
+  }
+  cm7_cp_wait_all();
+  __syncthreads();
+
+  // ---- phase 2: face tasks (trace -> s* - s^-) and line tasks, independent
+  for (int fn = THREADS - 1 - t; fn < 6 * NF; fn += THREADS) {
+    int f, m, d, s, nm, np_, kline;
+    cm7_face_node<Nq>(fn, f, m, d, s, nm, np_, kline);
+    double* tr = T + f * TS + m;
+    double dl[6];
+    if (!((pos.wallmask >> f) & 1)) {
+      double Yp[6], sp[6];
+#pragma unroll
+      for (int v = 0; v < NV; ++v) Yp[v] = tr[v * NF];
+      cm7_eos_grad<MOIST, RICH>(p, Yp, p.th.grav * tr[NV * NF], sp);
+#pragma unroll
+      for (int v = 0; v < NS; ++v) dl[v] = 0.5 * (sp[v] - ss[v * SLOT + nm]);
+    } else {
+      // wall: u_bc = u^- - (n.u^-) n  (A6), n along Ja^d of the wall node; scalars unchanged (A8)
+      const double A0 = geo[(3 * d) * SLOT + nm], A1 = geo[(3 * d + 1) * SLOT + nm], A2 = geo[(3 * d + 2) * SLOT + nm];
+      const double ua = (ss[nm] * A0 + ss[SLOT + nm] * A1 + ss[2 * SLOT + nm] * A2) / (A0 * A0 + A1 * A1 + A2 * A2);
+#pragma unroll
+      for (int v = 0; v < NS; ++v) dl[v] = 0.0;
+      dl[0] = -ua * A0; dl[1] = -ua * A1; dl[2] = -ua * A2;
+    }
+#pragma unroll
+    for (int v = 0; v < NS; ++v) tr[v * NF] = dl[v];
+  }
+  for (int lt = t; lt < 3 * NFP; lt += THREADS) {
+    const int d = lt / NFP, l = lt % NFP;
+    if (l < NF) {
+      if (d == 0) cm11_grad_line<Nq, NS, SLOT, 0>(p, ss, dd, l);
+      else if (d == 1) cm11_grad_line<Nq, NS, SLOT, 1>(p, ss, dd + NS * SLOT, l);
+      else cm11_grad_line<Nq, NS, SLOT, 2>(p, ss, dd + 2 * NS * SLOT, l);
+    }
+  }
+  __syncthreads();
+
+  // ---- phase 3: lifted jumps, physical gradient, closure, store
+  if (node) {
+    const size_t idx = (size_t)e * NP + n;
+    double dr[6][3];
+    const int c3[3] = {i_, j_, k_};
+    const int m3[3] = {j_ + Nq * k_, i_ + Nq * k_, i_ + Nq * j_};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+#pragma unroll
+      for (int v = 0; v < NS; ++v) dr[v][c] = dd[(c * NS + v) * SLOT + n];
+      if (c3[c] == 0 || c3[c] == N) {
+        const bool hi = (c3[c] == N);
+        const double* tr = T + (2 * c + (hi ? 1 : 0)) * TS + m3[c];
+        const double w = hi ? p.inv_w0 : -p.inv_w0;
+#pragma unroll
+        for (int v = 0; v < NS; ++v) dr[v][c] += w * tr[v * NF];
+      }
+    }
+    double Ja[3][3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) Ja[d][c] = geo[(3 * d + c) * SLOT + n];
+    const double invJ = geo[9 * SLOT + n];
+    double G[6][3];
+#pragma unroll
+    for (int v = 0; v < NS; ++v)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) G[v][c] = invJ * (Ja[0][c] * dr[v][0] + Ja[1][c] * dr[v][1] + Ja[2][c] * dr[v][2]);
+    double Gr[5][3];
+#pragma unroll
+    for (int v = 0; v < 5; ++v)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) Gr[v][c] = (v < NS0) ? G[v][c] : 0.0;
+    double* o = p.Gout + idx;
+    if (RAW) {
+#pragma unroll
+      for (int v = 0; v < 5; ++v)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) __stcs(o + (size_t)(3 * v + c) * p.stride, Gr[v][c]);
+    } else {
+      double thv = 1.0, dthv = 0.0;
+      if (RICH) { thv = ss[NS0 * SLOT + n]; dthv = G[NS0][2]; }
+      double g[12];
+      cm_closure<MOIST>(p, Gr, geo[11 * SLOT + n], geo[12 * SLOT + n], geo[13 * SLOT + n], geo[14 * SLOT + n], thv, dthv, g);
+#pragma unroll
+      for (int k = 0; k < C::NG; ++k) o[(size_t)k * p.stride] = g[k];
     }
   }
 }

@@ -180,6 +180,26 @@ cudaError_t launch_tend11(const CmKP& kp, cudaStream_t st) {
   return cudaGetLastError();
 }
 
+template <int Nq, bool MOIST, bool RAW, bool RICH>
+cudaError_t launch_grad11(const CmKP& kp, cudaStream_t st) {
+  using C = CmCfg7<Nq, MOIST>;
+  using R = CmCfg11G<Nq, MOIST, RICH>;
+  static LaunchState ls;
+  int wave = 0;
+  cudaError_t err = configure(cm11_gradient_kernel<Nq, MOIST, RAW, RICH>, R::SMEM, ls, C::THREADS, &wave);
+  if (err != cudaSuccess) return err;
+  CmKP k2 = kp;
+  if (k2.ahead < 0) k2.ahead = wave;
+  cm11_gradient_kernel<Nq, MOIST, RAW, RICH><<<dim3(kp.gPY * kp.gL, kp.gEz, kp.gNXC * kp.gNYP), C::THREADS, R::SMEM, st>>>(k2);
+  return cudaGetLastError();
+}
+
+template <int Nq, bool MOIST>
+cudaError_t launch_grad11m(const CmKP& kp, cudaStream_t st) {
+  if (kp.mode == 1) return launch_grad11<Nq, MOIST, true, false>(kp, st);
+  return kp.richardson ? launch_grad11<Nq, MOIST, false, true>(kp, st) : launch_grad11<Nq, MOIST, false, false>(kp, st);
+}
+
 template <int Nq, bool MOIST, bool SGS>
 cudaError_t launch_tend11m(const CmKP& kp, cudaStream_t st) {
   if (kp.mode == 0) return launch_tend11<Nq, MOIST, SGS, 0>(kp, st);
@@ -198,6 +218,9 @@ cudaError_t CM_CAT(cm_launch_gradient_nq, CM_NQ)(const CmKP& kp, int moist, int 
     }
     if (kp.richardson) return moist ? launch_grad7<CM_NQ, true, false, false, true>(kp, st) : launch_grad7<CM_NQ, false, false, false, true>(kp, st);
     return moist ? launch_grad7<CM_NQ, true, false>(kp, st) : launch_grad7<CM_NQ, false, false>(kp, st);
+  }
+  if constexpr (CmCfg11G<CM_NQ, true, true>::OK) {
+    if (variant == 11 && general) return moist ? launch_grad11m<CM_NQ, true>(kp, st) : launch_grad11m<CM_NQ, false>(kp, st);
   }
   if (moist) return general ? launch_grad2<CM_NQ, true, 1>(kp, st) : launch_grad2<CM_NQ, true, 0>(kp, st);
   return general ? launch_grad2<CM_NQ, false, 1>(kp, st) : launch_grad2<CM_NQ, false, 0>(kp, st);

@@ -372,10 +372,12 @@ __global__ void filter_kernel(const __grid_constant__ FilterArgs a) {
 
 // a6, second stage: the per-element partial sums are reduced on the device in a fixed order (thread t takes elements
 // t, t + T, ...; then a fixed tree), so only 7 doubles travel to the host
-__global__ void diag_reduce_kernel(long long Ne, const double* __restrict__ part, double* __restrict__ out) {
+__global__ void diag_reduce_kernel(long long n, long long chunk, const double* __restrict__ part, double* __restrict__ out) {
   __shared__ double sh[7][256];
   double r[7] = {0, 0, 0, 0, 0, 0, 0};
-  for (long long e = threadIdx.x; e < Ne; e += blockDim.x)
+  const long long e0 = blockIdx.x * chunk, e1 = (e0 + chunk < n) ? e0 + chunk : n;    // block b reduces entries [e0, e1)
+  out += 7 * blockIdx.x;
+  for (long long e = e0 + threadIdx.x; e < e1; e += blockDim.x)
     for (int m = 0; m < 7; ++m) { const double v = part[7 * e + m]; r[m] = (m == 5) ? fmax(r[m], v) : r[m] + v; }
   for (int m = 0; m < 7; ++m) sh[m][threadIdx.x] = r[m];
   __syncthreads();
@@ -514,8 +516,17 @@ struct cm_dg_ctx {
   int *d_nbr = nullptr, *d_erow = nullptr, *d_lex = nullptr;
   double *d_ztab = nullptr, *d_geo = nullptr, *d_ref = nullptr, *d_G = nullptr, *d_res = nullptr, *d_Q2 = nullptr, *d_Q3 = nullptr;
   double *d_zsfc = nullptr, *d_xyz_user = nullptr, *d_part = nullptr, *d_stage = nullptr;
-  double *d_lev = nullptr;         // [Ez*Nq][CM_DG_NPROF] level statistics + [Ez*Nq] sum of weights + 7 reduced diagnostics
+  double *d_lev = nullptr;         // [Ez*Nq][CM_DG_NPROF] level statistics + [Ez*Nq] sum of weights + 8 reduced diagnostics + [256][7] block results
   int tileL = 1, tilePY = 1;       // the tiled element order (x-chunk, y-patch)
+  // one time step as a CUDA graph: captured on the second consecutive call with the same state array, dt and coefficient
+  // table, replayed afterwards (the 10-12 launches of a step are launch-bound on small meshes)
+  struct StepKey {
+    const double* Q = nullptr; double dt = 0.0; int nstages = 0; double tab = 0.0;
+    bool operator==(const StepKey& o) const { return Q == o.Q && dt == o.dt && nstages == o.nstages && tab == o.tab; }
+  };
+  bool graphs = true;
+  cudaGraphExec_t step_exec = nullptr;
+  StepKey step_key, last_key;
   CmKP kp;
   cm_launch_fn launch_grad = nullptr, launch_tend = nullptr;
   int ahead_t = -1, ahead_g = -1;   // L2 prefetch distance of the tendency / gradient kernel (-1 = one wave)
@@ -534,6 +545,7 @@ void free_ctx(cm_dg_ctx* c) {
   cudaFree(c->d_ref); cudaFree(c->d_G); cudaFree(c->d_res); cudaFree(c->d_Q2); cudaFree(c->d_Q3); cudaFree(c->d_zsfc);
   cudaFree(c->d_xyz_user); cudaFree(c->d_part); cudaFree(c->d_stage); cudaFree(c->d_lev);
   for (auto e : c->ev) cudaEventDestroy(e);
+  if (c->step_exec) cudaGraphExecDestroy(c->step_exec);
   delete c;
 }
 
@@ -784,6 +796,7 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   for (int d = 0; d < 3; ++d) kp.gbc[d] = p->bc[d];
   kp.ahead = -1;   // L2 prefetch distance of the cm7 kernels: -1 = one wave of resident CTAs (set by the launcher)
   c->ahead_t = tn.ahead_t; c->ahead_g = tn.ahead_g;
+  c->graphs = tn.no_graph == 0;
   kp.gS = L;       // row-sweep kernels: a row is a whole x-chunk unless the mesh is small or the tuning asks for shorter rows
   {
     // small meshes: long rows leave too few CTAs for an even last wave (config 3 at 32x32x16: 512 rows of 32 on 444 CTA
@@ -909,7 +922,7 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   c->em_bytes_per_field = std::max(fbytes, (size_t)Ne * slot * sizeof(double));
   if (p->sgs) CM_CUDA_B(cudaMalloc(&c->d_G, (size_t)c->ngrad * c->em_bytes_per_field));
   CM_CUDA_B(cudaMalloc(&c->d_part, (size_t)Ne * 7 * sizeof(double)));
-  CM_CUDA_B(cudaMalloc(&c->d_lev, ((size_t)p->ne[2] * Nq * (CM_DG_NPROF + 1) + 8) * sizeof(double)));
+  CM_CUDA_B(cudaMalloc(&c->d_lev, ((size_t)p->ne[2] * Nq * (CM_DG_NPROF + 1) + 8 + 7 * 256) * sizeof(double)));
   // LSRK residual and the two further state buffers of the stage ring (cm_dg_lsrk_step never allocates or synchronises)
   {
     const size_t sb = (size_t)c->nvar * fbytes;
@@ -993,6 +1006,26 @@ int cm_dg_filter(cm_dg_ctx* ctx, double* Q_dev) {
   return CM_DG_OK;
 }
 
+// the launches of ONE time step on the ctx stream
+static int one_step(cm_dg_ctx* ctx, double* Q_dev, double dt, int nstages, const double* A, const double* B) {
+  const size_t bytes = (size_t)ctx->nvar * ctx->stride * sizeof(double);
+  // A stage never updates in place (neighbours still read the old state).  The stages cycle
+  // Q_dev -> Q2 -> Q3 -> Q2 -> ... -> Q_dev: the last stage of a step writes the caller's array, no copy is appended
+  // (a one-stage scheme writes Q2 and is copied back).
+  int rc;
+  double* src = Q_dev;
+  for (int st = 0; st < nstages; ++st) {
+    double* dst = (st == nstages - 1 && nstages > 1) ? Q_dev : ((st & 1) ? ctx->d_Q3 : ctx->d_Q2);
+    if (ctx->prm.sgs) { rc = run_gradient(ctx, src, ctx->d_G, 0); if (rc) return rc; }
+    rc = run_tendency(ctx, src, ctx->d_res, dst, 1, A[st], B[st], dt);
+    if (rc) return rc;
+    src = dst;
+  }
+  if (nstages == 1) CM_CUDA(cudaMemcpyAsync(Q_dev, ctx->d_Q2, bytes, cudaMemcpyDeviceToDevice, ctx->st));
+  if (ctx->prm.filter_order > 0) { rc = cm_dg_filter(ctx, Q_dev); if (rc) return rc; }
+  return CM_DG_OK;
+}
+
 int cm_dg_lsrk_step_table(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, int32_t nsteps, int32_t nstages,
                           const double* A, const double* B, const double* C) {
   (void)t; (void)C;   // no time-dependent forcing on this path (reading R14)
@@ -1000,22 +1033,40 @@ int cm_dg_lsrk_step_table(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, in
   if (nsteps < 0 || nstages < 1) return fail(CM_DG_EINVAL, "cm_dg_lsrk_step_table: nsteps must be >= 0 and nstages >= 1");
   if (A[0] != 0.0) return fail(CM_DG_EINVAL, "cm_dg_lsrk_step_table: A[0] must be 0 (the residual starts from zero)");
   int rc = enter(ctx, "cm_dg_lsrk_step_table"); if (rc) return rc;
-  const size_t bytes = (size_t)ctx->nvar * ctx->stride * sizeof(double);
-  // A stage never updates in place (neighbours still read the old state).  The stages cycle
-  // Q_dev -> Q2 -> Q3 -> Q2 -> ... -> Q_dev: the last stage of a step writes the caller's array, no copy is appended
-  // (a one-stage scheme writes Q2 and is copied back).
-  for (int s = 0; s < nsteps; ++s) {
-    double* src = Q_dev;
-    for (int st = 0; st < nstages; ++st) {
-      double* dst = (st == nstages - 1 && nstages > 1) ? Q_dev : ((st & 1) ? ctx->d_Q3 : ctx->d_Q2);
-      if (ctx->prm.sgs) { rc = run_gradient(ctx, src, ctx->d_G, 0); if (rc) return rc; }
-      rc = run_tendency(ctx, src, ctx->d_res, dst, 1, A[st], B[st], dt);
-      if (rc) return rc;
-      src = dst;
+  // CUDA graph of one step: every kernel argument (state pointers of the stage ring, dt, A_s, B_s) is fixed by
+  // (Q_dev, dt, table), so the step captured for that key can be replayed.  Captured on the second consecutive call with the
+  // same key (the first one has configured every kernel on this device); never while the per-launch events of
+  // cm_dg_profile_begin are on; any failure (e.g. the legacy default stream cannot be captured) falls back to plain launches.
+  if (ctx->graphs && !ctx->profiling && nsteps > 0) {
+    cm_dg_ctx::StepKey key;
+    key.Q = Q_dev; key.dt = dt; key.nstages = nstages;
+    for (int s = 0; s < nstages; ++s) key.tab += (s + 1) * (A[s] + 3.0 * B[s]);
+    if (ctx->step_exec && key == ctx->step_key) {
+      for (int s = 0; s < nsteps; ++s) CM_CUDA(cudaGraphLaunch(ctx->step_exec, ctx->st));
+      return CM_DG_OK;
     }
-    if (nstages == 1) CM_CUDA(cudaMemcpyAsync(Q_dev, ctx->d_Q2, bytes, cudaMemcpyDeviceToDevice, ctx->st));
-    if (ctx->prm.filter_order > 0) { rc = cm_dg_filter(ctx, Q_dev); if (rc) return rc; }
+    if (key == ctx->last_key) {
+      if (ctx->step_exec) { cudaGraphExecDestroy(ctx->step_exec); ctx->step_exec = nullptr; }
+      cudaGraph_t graph = nullptr;
+      if (cudaStreamBeginCapture(ctx->st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+        const int rs = one_step(ctx, Q_dev, dt, nstages, A, B);
+        const cudaError_t ee = cudaStreamEndCapture(ctx->st, &graph);
+        if (rs == CM_DG_OK && ee == cudaSuccess && graph && cudaGraphInstantiate(&ctx->step_exec, graph, 0) == cudaSuccess)
+          ctx->step_key = key;
+        else
+          ctx->step_exec = nullptr;
+        if (graph) cudaGraphDestroy(graph);
+      }
+      cudaGetLastError();                                  // a refused capture is not an error of this call
+      if (ctx->step_exec) {
+        for (int s = 0; s < nsteps; ++s) CM_CUDA(cudaGraphLaunch(ctx->step_exec, ctx->st));
+        return CM_DG_OK;
+      }
+      ctx->graphs = false;                                 // do not try again on this ctx
+    }
+    ctx->last_key = key;
   }
+  for (int s = 0; s < nsteps; ++s) { rc = one_step(ctx, Q_dev, dt, nstages, A, B); if (rc) return rc; }
   return CM_DG_OK;
 }
 
@@ -1039,8 +1090,12 @@ int cm_dg_diagnostics(cm_dg_ctx* ctx, const double* Q_dev, cm_dg_diag* out) {
   CM_CUDA(cudaGetLastError());
   double* d_red = ctx->d_lev + (size_t)ctx->prm.ne[2] * ctx->Nq * (CM_DG_NPROF + 1);
   {
+    // two fixed-order stages: 256 blocks over contiguous element ranges, then one block over their results
     Timed tm(ctx, 2);
-    diag_reduce_kernel<<<1, 256, 0, ctx->st>>>(ctx->Ne, ctx->d_part, d_red);
+    const int nb = 256;
+    const long long chunk = (ctx->Ne + nb - 1) / nb;
+    diag_reduce_kernel<<<nb, 256, 0, ctx->st>>>(ctx->Ne, chunk, ctx->d_part, d_red + 8);
+    diag_reduce_kernel<<<1, 256, 0, ctx->st>>>(nb, nb, d_red + 8, d_red);
   }
   CM_CUDA(cudaGetLastError());
   double s[7] = {0, 0, 0, 0, 0, 0, 0};
