@@ -107,6 +107,8 @@ typedef struct {
                             whole chunk on large meshes, shorter rows (>= 8) where that leaves fewer than 4 waves of CTAs   */
   int32_t no_graph;      /* 1: cm_dg_lsrk_step* always launch kernel by kernel; 0: a time step is captured as a CUDA graph on
                             the second consecutive call with the same (Q_dev, dt, table) and replayed afterwards           */
+  int32_t no_terrain;    /* 1: a terrain-following mesh (geom == 1) is treated like any stored-metric mesh (nine metric tiles
+                            per element instead of the three that such a mesh needs)                                       */
 } cm_dg_tuning;
 
 /* Conservation integrals and step-size ingredients (eq. 57; eq. 61-62). */

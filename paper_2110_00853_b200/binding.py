@@ -34,7 +34,7 @@ class _Params(C.Structure):
 class _Tuning(C.Structure):
     _fields_ = [("order_lex", C.c_int32), ("max_chunk", C.c_int32), ("max_patch", C.c_int32), ("force_general", C.c_int32),
                 ("kernel", C.c_int32), ("ahead_t", C.c_int32), ("ahead_g", C.c_int32), ("row_len", C.c_int32),
-                ("no_graph", C.c_int32)]
+                ("no_graph", C.c_int32), ("no_terrain", C.c_int32)]
 
 
 class _Diag(C.Structure):

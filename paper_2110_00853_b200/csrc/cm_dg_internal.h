@@ -37,6 +37,7 @@ struct CmKP {
   int richardson;        // eq. (40): nu_t *= f_b (one more gradient variable, theta_v)
   int riemann;           // 0 Rusanov | 1 HLLC | 2 Roe (stored-metric kernels)
   int use_ref;           // reference state removed (R12) or plain pressure
+  int terrain;           // stored-metric meshes: 1 = terrain-following (geom == 1): Ja^1, Ja^2 axis-aligned (cm_dg_kernels11.cuh)
   int satadj;            // 1: temperature and liquid water from the saturation adjustment of eq. (15) (stored-metric kernels)
   int mode;              // tendency: 0 dQ := rhs | 1 LSRK stage.  gradient: 0 packed SGS fluxes | 1 raw 15 gradients
   // arrays

@@ -20,10 +20,27 @@
 #pragma once
 #include "cm_dg_kernels7.cuh"
 
-template <int Nq, bool MOIST, bool SGS, int MODE> struct CmCfg11 {
+// TERR: terrain-following mesh (geom == 1: x and y stay a uniform brick, only z is warped).  Then
+//   Ja^1 = (h_y/2 z_zeta, 0, 0),  Ja^2 = (0, h_x/2 z_zeta, 0),  Ja^3 = (-h_y/2 z_xi, -h_x/2 z_eta, h_x h_y/4)      (eq. 24)
+// and three of the nine metric tiles carry everything: Ja[0], Ja[6], Ja[7] (Ja[4] = Ja[0] h_x/h_y, Ja[8] is a constant).
+template <bool TERR> struct Cm11Geo {
+  static constexpr int NGEO = TERR ? 6 : 12;            // tiles: Ja (9 | 3), 1/J, z, tau_s
+  static constexpr int S_INVJ = NGEO - 3, S_Z = NGEO - 2, S_TAUS = NGEO - 1;
+  __host__ __device__ static constexpr int field(int k) {   // tile k of the geometry block -> CmKP::geo field
+    return TERR ? (k == 0 ? 0 : k == 1 ? 6 : k == 2 ? 7 : k == 3 ? 9 : k == 4 ? 10 : 15) : (k < 11 ? k : 15);
+  }
+  // metric entry Ja[m] (m = 3 d + c, compile-time in unrolled code) of node n; r = h_x / h_y, a3 = h_x h_y / 4
+  template <int SLOT>
+  __device__ __forceinline__ static double ja(const double* __restrict__ geo, int m, int n, double r, double a3) {
+    if (!TERR) return geo[m * SLOT + n];
+    return (m == 0) ? geo[n] : (m == 4) ? geo[n] * r : (m == 6) ? geo[SLOT + n] : (m == 7) ? geo[2 * SLOT + n] : (m == 8) ? a3 : 0.0;
+  }
+};
+
+template <int Nq, bool MOIST, bool SGS, int MODE, bool TERR = false> struct CmCfg11 {
   using C = CmCfg7<Nq, MOIST>;
   static constexpr int NF = C::NF, NP = C::NP, NV = C::NV, NG = SGS ? C::NG : 0, SLOT = C::SLOT, THREADS = C::THREADS;
-  static constexpr int NGEO = 12;                       // Ja 9, 1/J, z, tau_s  (fields 0..8, 9, 10, 15 of CmKP::geo)
+  static constexpr int NGEO = Cm11Geo<TERR>::NGEO;      // fields 0..8, 9, 10, 15 of CmKP::geo, or 0, 6, 7, 9, 10, 15
   static constexpr int NREF = MOIST ? 3 : 2;            // rho_r, rhoe_r, [rhoq_r]
   static constexpr int NTR = NV + NG + 1 + NREF;        // trace values per face node: state, SGS fluxes, z, reference
   static constexpr int TS = C::fstride(NTR);
@@ -42,17 +59,16 @@ template <int Nq, bool MOIST, bool SGS, int MODE> struct CmCfg11 {
   static constexpr int MINB = C::cap(C::fit(SMEM), C::cap(640 / THREADS, 16));
 };
 
-__host__ __device__ constexpr int cm11_geo_field(int k) { return k < 11 ? k : 15; }   // tile k of the geometry block -> CmKP::geo field
-
 // face task on a stored-metric mesh: replaces the trace of face node fn by
 //   rf[v] = -(1/2) A.F^+[v] - (1/2) sJ lambda (Y^-[v] - Y^+[v])     interior / periodic (eq. 27 with R1, R2; P:L274 with R6)
 //   rf    = [0; -(p' + rho u_n (u_n + lambda)) A; 0; 0] + surface fluxes on the bottom wall      free-slip wall (A6-A7, R10)
 // with A = +-Ja^d of the own face node (outward, |A| = sJ)
-template <int Nq, bool MOIST, bool SGS, int MODE>
+template <int Nq, bool MOIST, bool SGS, int MODE, bool TERR>
 __device__ __forceinline__ void cm11_tend_face(const CmKP& p, const double* __restrict__ Qs, const double* __restrict__ cs,
                                                const double* __restrict__ geo, const double* __restrict__ ref, double* __restrict__ T,
                                                int wallmask, int fn) {
-  using R = CmCfg11<Nq, MOIST, SGS, MODE>;
+  using R = CmCfg11<Nq, MOIST, SGS, MODE, TERR>;
+  using GG = Cm11Geo<TERR>;
   constexpr int NF = R::NF, NV = R::NV, NG = R::NG, SLOT = R::SLOT, TS = R::TS, NREF = R::NREF;
   int f, m, d, s, nm, np_, kline;
   cm7_face_node<Nq>(fn, f, m, d, s, nm, np_, kline);
@@ -60,8 +76,15 @@ __device__ __forceinline__ void cm11_tend_face(const CmKP& p, const double* __re
   double* tr = T + f * TS + m;
   const double sgn = s ? 1.0 : -1.0;
   double A[3];
+  if (TERR) {
+    const double r = p.cA[1] * cm_rcp(p.cA[0]), a0 = geo[nm];
+    A[0] = sgn * ((d == 0) ? a0 : (d == 1) ? 0.0 : geo[SLOT + nm]);
+    A[1] = sgn * ((d == 0) ? 0.0 : (d == 1) ? a0 * r : geo[2 * SLOT + nm]);
+    A[2] = sgn * ((d == 2) ? p.cA[2] : 0.0);
+  } else {
 #pragma unroll
-  for (int c = 0; c < 3; ++c) A[c] = sgn * geo[(3 * d + c) * SLOT + nm];
+    for (int c = 0; c < 3; ++c) A[c] = sgn * geo[(3 * d + c) * SLOT + nm];
+  }
   const double sJ = cm_sqrt(A[0] * A[0] + A[1] * A[1] + A[2] * A[2]);
   double Ym[6];
 #pragma unroll
@@ -93,7 +116,7 @@ __device__ __forceinline__ void cm11_tend_face(const CmKP& p, const double* __re
 #pragma unroll
     for (int v = 0; v < NV; ++v) rf[v] = -0.5 * Fp[v] - 0.5 * lamsJ * (Ym[v] - Yp[v]);
   } else {
-    st.Phi = p.th.grav * geo[10 * SLOT + nm]; st.taus = 0.0;
+    st.Phi = p.th.grav * geo[GG::S_Z * SLOT + nm]; st.taus = 0.0;
     if (p.use_ref) {
       st.rho_r = ref[nm]; st.rhoe_r = ref[SLOT + nm];
       st.rhoq_r = MOIST ? ref[2 * SLOT + nm] : 0.0;
@@ -115,10 +138,11 @@ __device__ __forceinline__ void cm11_tend_face(const CmKP& p, const double* __re
 }
 
 // MODE: 0 dQ := rhs | 1 LSRK stage reading the residual | 2 LSRK stage with A_s = 0 (residual not read)
-template <int Nq, bool MOIST, bool SGS, int MODE>
-__global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg11<Nq, MOIST, SGS, MODE>::MINB) cm11_tendency_kernel(const __grid_constant__ CmKP p) {
+template <int Nq, bool MOIST, bool SGS, int MODE, bool TERR>
+__global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg11<Nq, MOIST, SGS, MODE, TERR>::MINB) cm11_tendency_kernel(const __grid_constant__ CmKP p) {
   using C = CmCfg7<Nq, MOIST>;
-  using R = CmCfg11<Nq, MOIST, SGS, MODE>;
+  using R = CmCfg11<Nq, MOIST, SGS, MODE, TERR>;
+  using GG = Cm11Geo<TERR>;
   constexpr int NF = C::NF, NP = C::NP, N = Nq - 1, NV = C::NV, NG = R::NG, SLOT = C::SLOT, NFP = C::NFP, THREADS = C::THREADS;
   constexpr int TS = R::TS, NREF = R::NREF, NGEO = R::NGEO;
   extern __shared__ __align__(128) double smem11[];
@@ -162,7 +186,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg11<Nq, MOIST,
     {
       uint32_t d = cm7_saddr(Gt);
 #pragma unroll
-      for (int k = 0; k < NGEO; ++k) { cm7_bulk_g2s_raw(d, p.geo + (size_t)cm11_geo_field(k) * p.stride + src, SLOT * 8, mb); d += SLOT * 8; }
+      for (int k = 0; k < NGEO; ++k) { cm7_bulk_g2s_raw(d, p.geo + (size_t)GG::field(k) * p.stride + src, SLOT * 8, mb); d += SLOT * 8; }
     }
     {
       uint32_t d = cm7_saddr(Ht);
@@ -178,7 +202,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg11<Nq, MOIST,
       if (k < NV) g = p.Q + (size_t)k * p.stride;
       else if ((k -= NV) < NG) g = p.G + (size_t)k * p.stride;
       else if ((k -= NG) < (MODE == 1 ? NV : 0)) g = p.dQ + (size_t)k * p.stride;
-      else if ((k -= (MODE == 1 ? NV : 0)) < NGEO) g = p.geo + (size_t)cm11_geo_field(k) * p.stride;
+      else if ((k -= (MODE == 1 ? NV : 0)) < NGEO) g = p.geo + (size_t)GG::field(k) * p.stride;
       else g = p.ref + (size_t)(k - NGEO) * p.stride;
       cm7_prefetch_l2(g + src, SLOT * 8);
     }
@@ -223,11 +247,12 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg11<Nq, MOIST,
     if (SGS)
 #pragma unroll
       for (int k = 0; k < NG; ++k) g[k] = Fs[k * SLOT + n];
+    const double hr = TERR ? p.cA[1] * cm_rcp(p.cA[0]) : 0.0;
     double Ja[9];
 #pragma unroll
-    for (int m = 0; m < 9; ++m) Ja[m] = geo[m * SLOT + n];
-    invJ = geo[9 * SLOT + n]; taus = geo[11 * SLOT + n];
-    st.Phi = p.th.grav * geo[10 * SLOT + n]; st.taus = taus;
+    for (int m = 0; m < 9; ++m) Ja[m] = GG::template ja<SLOT>(geo, m, n, hr, p.cA[2]);
+    invJ = geo[GG::S_INVJ * SLOT + n]; taus = geo[GG::S_TAUS * SLOT + n];
+    st.Phi = p.th.grav * geo[GG::S_Z * SLOT + n]; st.taus = taus;
     if (p.use_ref) {
       st.rho_r = ref[n]; st.rhoe_r = ref[SLOT + n];
       st.rhoq_r = MOIST ? ref[2 * SLOT + n] : 0.0;
@@ -239,8 +264,13 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg11<Nq, MOIST,
     buoy = P.drho * p.th.grav;
     cs[n] = cm_sqrt(P.c2);
     double Fa[6], Fb[6], Fc[6];
-    cm_flux_dir<MOIST>(Y, P, SGS, g, Ja[0], Ja[1], Ja[2], Fa);
-    cm_flux_dir<MOIST>(Y, P, SGS, g, Ja[3], Ja[4], Ja[5], Fb);
+    if (TERR) {                                        // Ja^1, Ja^2 are axis-aligned
+      cm_flux_axis<MOIST, 0>(Y, P, SGS, g, Ja[0], Fa);
+      cm_flux_axis<MOIST, 1>(Y, P, SGS, g, Ja[4], Fb);
+    } else {
+      cm_flux_dir<MOIST>(Y, P, SGS, g, Ja[0], Ja[1], Ja[2], Fa);
+      cm_flux_dir<MOIST>(Y, P, SGS, g, Ja[3], Ja[4], Ja[5], Fb);
+    }
     cm_flux_dir<MOIST>(Y, P, SGS, g, Ja[6], Ja[7], Ja[8], Fc);
 #pragma unroll
     for (int v = 0; v < NV; ++v) { Fs[v * SLOT + n] = Fa[v]; Fs[(NV + v) * SLOT + n] = Fc[v]; F2[v * C::SLOT2 + n2] = Fb[v]; }
@@ -255,7 +285,7 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS, CmCfg11<Nq, MOIST,
     else { if (l < NF) cm7_tend_line<Nq, NV, SLOT, NF, 2>(p, Fs + NV * SLOT + l, pos.wallmask); }
   }
   cm7_cp_wait_all();                                   // this thread's trace copies have landed
-  for (int fn = THREADS - 1 - t; fn < 6 * NF; fn += THREADS) cm11_tend_face<Nq, MOIST, SGS, MODE>(p, Qs, cs, geo, ref, T, pos.wallmask, fn);
+  for (int fn = THREADS - 1 - t; fn < 6 * NF; fn += THREADS) cm11_tend_face<Nq, MOIST, SGS, MODE, TERR>(p, Qs, cs, geo, ref, T, pos.wallmask, fn);
   __syncthreads();
 
   // ---- phase 3: assemble the tendency of the own node and update

@@ -166,17 +166,17 @@ cudaError_t launch_tend10m(const CmKP& kp, cudaStream_t st) {
 }
 
 // CTA-per-element tendency kernel of stored-metric meshes (cm_dg_kernels11.cuh): grid = the tiled element order
-template <int Nq, bool MOIST, bool SGS, int MODE>
+template <int Nq, bool MOIST, bool SGS, int MODE, bool TERR>
 cudaError_t launch_tend11(const CmKP& kp, cudaStream_t st) {
   using C = CmCfg7<Nq, MOIST>;
-  using R = CmCfg11<Nq, MOIST, SGS, MODE>;
+  using R = CmCfg11<Nq, MOIST, SGS, MODE, TERR>;
   static LaunchState ls;
   int wave = 0;
-  cudaError_t err = configure(cm11_tendency_kernel<Nq, MOIST, SGS, MODE>, R::SMEM, ls, C::THREADS, &wave);
+  cudaError_t err = configure(cm11_tendency_kernel<Nq, MOIST, SGS, MODE, TERR>, R::SMEM, ls, C::THREADS, &wave);
   if (err != cudaSuccess) return err;
   CmKP k2 = kp;
   if (k2.ahead < 0) k2.ahead = wave;
-  cm11_tendency_kernel<Nq, MOIST, SGS, MODE><<<dim3(kp.gPY * kp.gL, kp.gEz, kp.gNXC * kp.gNYP), C::THREADS, R::SMEM, st>>>(k2);
+  cm11_tendency_kernel<Nq, MOIST, SGS, MODE, TERR><<<dim3(kp.gPY * kp.gL, kp.gEz, kp.gNXC * kp.gNYP), C::THREADS, R::SMEM, st>>>(k2);
   return cudaGetLastError();
 }
 
@@ -200,10 +200,15 @@ cudaError_t launch_grad11m(const CmKP& kp, cudaStream_t st) {
   return kp.richardson ? launch_grad11<Nq, MOIST, false, true>(kp, st) : launch_grad11<Nq, MOIST, false, false>(kp, st);
 }
 
+template <int Nq, bool MOIST, bool SGS, bool TERR>
+cudaError_t launch_tend11t(const CmKP& kp, cudaStream_t st) {
+  if (kp.mode == 0) return launch_tend11<Nq, MOIST, SGS, 0, TERR>(kp, st);
+  return (kp.rka != 0.0) ? launch_tend11<Nq, MOIST, SGS, 1, TERR>(kp, st) : launch_tend11<Nq, MOIST, SGS, 2, TERR>(kp, st);
+}
+
 template <int Nq, bool MOIST, bool SGS>
-cudaError_t launch_tend11m(const CmKP& kp, cudaStream_t st) {
-  if (kp.mode == 0) return launch_tend11<Nq, MOIST, SGS, 0>(kp, st);
-  return (kp.rka != 0.0) ? launch_tend11<Nq, MOIST, SGS, 1>(kp, st) : launch_tend11<Nq, MOIST, SGS, 2>(kp, st);
+cudaError_t launch_tend11m(const CmKP& kp, cudaStream_t st) {   // terrain-following meshes: three metric tiles instead of nine
+  return kp.terrain ? launch_tend11t<Nq, MOIST, SGS, true>(kp, st) : launch_tend11t<Nq, MOIST, SGS, false>(kp, st);
 }
 
 }  // namespace
@@ -235,7 +240,7 @@ cudaError_t CM_CAT(cm_launch_tendency_nq, CM_NQ)(const CmKP& kp, int moist, int 
     if (kp.sgs) return moist ? launch_tend7m<CM_NQ, true, true>(kp, st) : launch_tend7m<CM_NQ, false, true>(kp, st);
     return moist ? launch_tend7m<CM_NQ, true, false>(kp, st) : launch_tend7m<CM_NQ, false, false>(kp, st);
   }
-  if constexpr (CmCfg11<CM_NQ, true, true, 1>::OK) {   // one predicate per order
+  if constexpr (CmCfg11<CM_NQ, true, true, 1, false>::OK) {   // one predicate per order
     if (variant == 11 && general) {
       if (kp.sgs) return moist ? launch_tend11m<CM_NQ, true, true>(kp, st) : launch_tend11m<CM_NQ, false, true>(kp, st);
       return moist ? launch_tend11m<CM_NQ, true, false>(kp, st) : launch_tend11m<CM_NQ, false, false>(kp, st);

@@ -821,6 +821,7 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   }
   kp.Ne = (int)Ne; kp.stride = c->stride; kp.sgs = p->sgs; kp.use_ref = p->use_ref ? 1 : 0;
   kp.richardson = p->richardson; kp.riemann = p->riemann;
+  kp.terrain = (p->geom == 1 && p->metric_form == 0 && !tn.no_terrain) ? 1 : 0;
   kp.cs2 = p->C_s * p->C_s;
   for (int d = 0; d < 3; ++d) { kp.d2[d] = (c->h[d] / c->N) * (c->h[d] / c->N); kp.urelax[d] = p->u_relax[d]; }
   kp.th.p_0 = c->prm.p_0; kp.th.kap_pd = p->R_d / (p->c_vd + p->R_d); kp.th.iRd = 1.0 / p->R_d;
