@@ -288,14 +288,14 @@ LEGS = {
 def one_leg(P, torch, name, peak):
     """One of the further workloads by name (also `bench.py --leg NAME`, the command the ncu captures of the stored-metric
     kernels run).  For the stored-metric legs the bytes those kernels really move are reported beside the algorithmic
-    ones: they read 12 geometry fields (Ja 9, 1/J, z, tau_s) and 2 reference fields per node that the 2.5-D-specialised
-    count of SURVEY 8(d) replaces by 5 values."""
+    ones: on a terrain-following mesh the tendency kernel reads 6 geometry fields (Ja^1_x, Ja^3_x, Ja^3_y, 1/J, z, tau_s) and
+    2 reference fields per node where the 2.5-D-specialised count of SURVEY 8(d) has 5 values."""
     import workloads as W
     make, steps, label, sb = LEGS[name]
     cfg, Q, dt = make(W)
     out = bench_leg(P, torch, cfg, Q, dt, steps, peak, label, stage_bytes(*sb))
     if sb[2]:
-        moved = (5 + 5 + 5 + 5 - 1.0) * 8 + (12 + 2) * 8          # Q, residual (4 of 5 stages), residual out, Q out + geometry + reference
+        moved = (5 + 5 + 5 + 5 - 1.0) * 8 + (6 + 2) * 8           # Q, residual (4 of 5 stages), residual out, Q out + geometry + reference
         if sb[1]:
             moved += (5 + 15 + 9) * 8 + 9 * 8                     # gradient sweep: Q, 15 geometry fields, G out; G read by the tendency
         out["moved_bytes_per_node_stage"] = moved
