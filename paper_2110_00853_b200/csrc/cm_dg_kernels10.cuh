@@ -40,18 +40,20 @@ template <int Nq, bool MOIST, int MODE> struct CmCfg10 {
   static constexpr int OFF_T = OFF_F2 + NV * C::SLOT2 + (NV * C::SLOT2 & 1);   // [NTB][4][TS]   eta / zeta neighbour traces, then rf
   static constexpr int TAILD = 3 * ((NTR * NF + 1) & ~1) + C::ZR * C::ZW + 6;   // xi blocks, z rows, mbarriers
   static constexpr size_t smem_with(int ntb) { return sizeof(double) * (size_t)(OFF_T + ntb * 4 * TS + TAILD); }
+#ifndef CM_R_REGTHREADS
+#define CM_R_REGTHREADS 512
+#endif
+  // resident CTAs the register budget allows (128 registers per thread at 512 threads per SM)
+  static constexpr int REGCAP = C::cap(CM_R_REGTHREADS / (C::THREADS + 32), 16);
   // the trace buffer is double-buffered (gathers issued one element ahead) when that costs no resident CTA
-  static constexpr int NTB = (C::fit(smem_with(2)) == C::fit(smem_with(1))) ? 2 : 1;
+  static constexpr int NTB = (C::cap(C::fit(smem_with(2)), REGCAP) == C::cap(C::fit(smem_with(1)), REGCAP)) ? 2 : 1;
   static constexpr int OFF_X = OFF_T + NTB * 4 * TS;                   // [3][XS]           xi- carry (x2), xi+ trace / rf
   static constexpr int OFF_Z = OFF_X + 3 * XS;                         // [ZR][ZW]          z rows
   static constexpr int OFF_M = OFF_Z + C::ZR * C::ZW;                  // mbarriers: tile buffer 0, 1, residual, gathered traces (x2), xi+ end trace
   static constexpr int DOUBLES = OFF_M + 6;
   static constexpr size_t SMEM = sizeof(double) * DOUBLES;
   static constexpr bool OK = SMEM <= 115712;                           // at least two CTAs per SM, else the cm7 kernels serve the order
-#ifndef CM_R_REGTHREADS
-#define CM_R_REGTHREADS 512
-#endif
-  static constexpr int MINB = C::cap(C::fit(SMEM), C::cap(CM_R_REGTHREADS / (C::THREADS + 32), 16));
+  static constexpr int MINB = C::cap(C::fit(SMEM), REGCAP);
 };
 
 // position of the CTA's row in the tiled library order: grid = (PY * NSEG, Ez, (Ey/PY) * (Ex/L)), NSEG = L / S rows per
