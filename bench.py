@@ -244,11 +244,11 @@ def stage_bytes(nvar, sgs, warped25):
     return grad + tend + geo
 
 
-def bench_leg(P, torch, cfg, Q, dt, steps, peak, label, bytes_per_node_stage):
+def bench_leg(P, torch, cfg, Q, dt, steps, peak, label, bytes_per_node_stage, tuning=None):
     """K LSRK54 steps of one further workload on the library stream, CUDA events; returns a small report dict."""
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
-        g = P.CmDg(cfg, stream=stream)
+        g = P.CmDg(cfg, stream=stream, tuning=tuning)
         Qd = torch.from_numpy(g.pack(Q)).to(g.device, non_blocking=False)
     stream.synchronize()
     nodes = g.n_elem * g.np
@@ -285,7 +285,7 @@ LEGS = {
 }
 
 
-def one_leg(P, torch, name, peak):
+def one_leg(P, torch, name, peak, tuning=None):
     """One of the further workloads by name (also `bench.py --leg NAME`, the command the ncu captures of the stored-metric
     kernels run).  For the stored-metric legs the bytes those kernels really move are reported beside the algorithmic
     ones: on a terrain-following mesh the tendency kernel reads 6 geometry fields (Ja^1_x, Ja^3_x, Ja^3_y, 1/J, z, tau_s) and
@@ -293,8 +293,10 @@ def one_leg(P, torch, name, peak):
     import workloads as W
     make, steps, label, sb = LEGS[name]
     cfg, Q, dt = make(W)
-    out = bench_leg(P, torch, cfg, Q, dt, steps, peak, label, stage_bytes(*sb))
-    if sb[2]:
+    out = bench_leg(P, torch, cfg, Q, dt, steps, peak, label, stage_bytes(*sb), tuning)
+    if tuning:
+        out["tuning"] = tuning
+    if sb[2] and not tuning:
         moved = (5 + 5 + 5 + 5 - 1.0) * 8 + (6 + 2) * 8           # Q, residual (4 of 5 stages), residual out, Q out + geometry + reference
         if sb[1]:
             moved += (5 + 15 + 9) * 8 + 9 * 8                     # gradient sweep: Q, 15 geometry fields, G out; G read by the tendency
@@ -502,7 +504,7 @@ def main():
     elif args.leg:
         import torch
         import paper_2110_00853_b200 as P
-        print(json.dumps(one_leg(P, torch, args.leg, measured_peaks()[0])))
+        print(json.dumps(one_leg(P, torch, args.leg, measured_peaks()[0], args.tuning)))
     elif args.impl == "reference":
         run_reference(args)
     else:
