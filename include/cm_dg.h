@@ -177,6 +177,50 @@ int cm_dg_filter(cm_dg_ctx* ctx, double* Q_dev);
 /* a6: conservation integrals etc. of Q_dev into *out_host; synchronises the stream. */
 int cm_dg_diagnostics(cm_dg_ctx* ctx, const double* Q_dev, cm_dg_diag* out_host);
 
+/* a6 without a ctx and without any device allocation.
+ *
+ * Who this is for: code that holds a state array on the GPU but is not in a position to obtain device memory through
+ * the CUDA allocator, and therefore cannot call cm_dg_setup (which cudaMallocs geometry, gradient and stage buffers).
+ * Typical cases: (1) a host application whose memory pool (a framework's caching allocator, an RMM-style arena) has
+ * already claimed the whole device, so a raw cudaMalloc beside it fails or eats into the pool's head-room; (2) a
+ * monitoring tool attached to a running model (for instance through CUDA IPC handles, or under an MPS memory limit) with
+ * no memory budget of its own; (3) a time loop that must not stall, because cudaMalloc and cudaFree synchronise the whole
+ * device.  For them the per-element partial sums of the conservation integrals live in ONE array that is compiled into
+ * the library (`static __device__`, CM_DG_STATIC_SCRATCH_BYTES = 3 684 416 bytes).  Every GPU on which the library's
+ * device code gets loaded holds that array until the process exits, whether or not this function is ever called.
+ *
+ * What it computes: the same sums as cm_dg_diagnostics (eq. 57; eq. 61-62) with the dry / unsaturated
+ * equation of state (eq. 6-10; no saturation adjustment), from arrays the caller provides in the library's layout:
+ *   Q_dev  DEVICE [nvar][field_stride]   state
+ *   J_dev  DEVICE [n_elem * np]          det(dx/dxi) per node (what cm_dg_metrics writes to J_dev)
+ *   z_dev  DEVICE [n_elem * np]          height of every node [m], Phi = grav * z (row 2 of what cm_dg_coords writes)
+ * The element order is irrelevant to these sums.  out_host (HOST) receives the result; min_node_dx is set to 0 (this call
+ * does not know the mesh).  `cuda_stream` is a cudaStream_t (NULL = default stream); the call synchronises it.
+ *
+ * Limits and rules:
+ *   - n_elem <= CM_DG_STATIC_MAX_ELEM; a larger mesh is refused with CM_DG_EINVAL and a message that names the limit
+ *     (nothing is launched).  N in 1..7, nvar 5 or 6, field_stride >= n_elem * (N+1)^3.
+ *   - It never calls cudaMalloc, cudaFree or any allocating library routine; the only device memory it writes is the
+ *     built-in array.  The result reaches the host by one 56-byte cudaMemcpyAsync.
+ *   - The first call on each device (with that device current) looks up the device address of the built-in array
+ *     (cudaGetSymbolAddress) and remembers it; later calls on that device reuse it.  Make that first call before any
+ *     stream capture is started on the device.
+ *   - All calls on one device share the array, and it keeps whatever the previous call left there.  Nothing in it has
+ *     to start at zero: every entry a call reads (n_elem x 7 partial sums, 256 x 7 block sums, 7 totals) is written
+ *     earlier in the same call, so a smaller mesh after a larger one never sees stale sums.  Two calls that overlap on
+ *     the same GPU (two streams, two host threads, two ctx-free users in one process) race on it: serialise them. */
+#define CM_DG_STATIC_MAX_ELEM 65536
+#define CM_DG_STATIC_SCRATCH_BYTES ((8 + 7 * 256 + 7 * CM_DG_STATIC_MAX_ELEM) * 8)
+typedef struct {
+  int32_t N;                 /* polynomial order, 1..7                                                      */
+  int32_t nvar;              /* 5 dry | 6 with rho*q_tot                                                    */
+  int64_t n_elem;            /* elements in Q_dev, 1..CM_DG_STATIC_MAX_ELEM                                 */
+  int64_t field_stride;      /* doubles between consecutive fields of Q_dev                                 */
+  double R_d, c_vd, R_v, c_vv, T_0, I_v0, grav; /* as in cm_dg_params                                       */
+} cm_dg_static_desc;
+int cm_dg_diagnostics_static(const cm_dg_static_desc* desc, const double* Q_dev, const double* J_dev, const double* z_dev,
+                             void* cuda_stream, cm_dg_diag* out_host);
+
 /* Density-weighted horizontal statistics of App. B (eq. B1-B4) on the nodal mesh.  Levels are the nodal
  * zeta-planes of every element layer, l = ez * Nq + k (nlev = Ez * Nq; the two planes of an element interface are separate
  * levels); <a>_l = sum W a / sum W over the plane with W = w_i w_j |Ja^3| (area element of the zeta = const surface).

@@ -43,13 +43,19 @@ class _Diag(C.Structure):
                 ("n_nonfinite", C.c_int64)]
 
 
+class _StaticDesc(C.Structure):
+    _fields_ = [("N", C.c_int32), ("nvar", C.c_int32), ("n_elem", C.c_int64), ("field_stride", C.c_int64),
+                ("R_d", C.c_double), ("c_vd", C.c_double), ("R_v", C.c_double), ("c_vv", C.c_double),
+                ("T_0", C.c_double), ("I_v0", C.c_double), ("grav", C.c_double)]
+
+
 class _KStats(C.Structure):
     _fields_ = [("launches_gradient", C.c_int64), ("launches_tendency", C.c_int64), ("launches_other", C.c_int64),
                 ("ms_gradient", C.c_double), ("ms_tendency", C.c_double), ("ms_other", C.c_double)]
 
 
 EXPORTS = ("cm_dg_setup", "cm_dg_setup_tuned", "cm_dg_layout", "cm_dg_coords", "cm_dg_metrics", "cm_dg_gradient", "cm_dg_rhs",
-           "cm_dg_lsrk_step", "cm_dg_lsrk_step_table", "cm_dg_filter", "cm_dg_diagnostics", "cm_dg_profiles", "cm_dg_rhs_host", "cm_dg_lsrk_step_host",
+           "cm_dg_lsrk_step", "cm_dg_lsrk_step_table", "cm_dg_filter", "cm_dg_diagnostics", "cm_dg_diagnostics_static", "cm_dg_profiles", "cm_dg_rhs_host", "cm_dg_lsrk_step_host",
            "cm_dg_profile_begin", "cm_dg_profile_end", "cm_dg_destroy", "cm_dg_last_error")
 
 _lib = None
@@ -79,6 +85,7 @@ def _load():
     L.cm_dg_lsrk_step_table.argtypes = [vp, vp, dbl, dbl, i32, i32, vp, vp, vp]
     L.cm_dg_filter.argtypes = [vp, vp]
     L.cm_dg_diagnostics.argtypes = [vp, vp, C.POINTER(_Diag)]
+    L.cm_dg_diagnostics_static.argtypes = [C.POINTER(_StaticDesc), vp, vp, vp, vp, C.POINTER(_Diag)]
     L.cm_dg_profiles.argtypes = [vp, vp, vp, i32]
     L.cm_dg_rhs_host.argtypes = [vp, vp, vp, dbl]
     L.cm_dg_lsrk_step_host.argtypes = [vp, vp, dbl, dbl, i32]
@@ -217,6 +224,23 @@ def cm_dg_diagnostics(ctx, Q_dev):
     d = _Diag()
     _check(_load().cm_dg_diagnostics(ctx, _dptr(Q_dev), C.byref(d)), "cm_dg_diagnostics")
     return {k: getattr(d, k) for k, _ in _Diag._fields_}
+
+
+STATIC_MAX_ELEM = 65536   # CM_DG_STATIC_MAX_ELEM
+
+
+def cm_dg_diagnostics_static(cfg, n_elem, field_stride, Q_dev, J_dev, z_dev, stream=None):
+    """Conservation sums of Q_dev without a ctx and without device allocation (include/cm_dg.h: for callers that cannot
+    cudaMalloc, e.g. beside a memory pool that owns the GPU).  cfg supplies N, nvar and the Table-1 constants; J_dev and z_dev
+    are per-node arrays in the library layout (cm_dg_metrics' J, row 2 of cm_dg_coords).  Marshalling only."""
+    d = _StaticDesc(N=int(cfg["N"]), nvar=int(cfg.get("nvar", 5)), n_elem=int(n_elem), field_stride=int(field_stride))
+    for k in ("R_d", "c_vd", "R_v", "c_vv", "T_0", "I_v0", "grav"):
+        setattr(d, k, float(cfg[k]))
+    out = _Diag()
+    sp = C.c_void_p(int(stream.cuda_stream)) if stream is not None else C.c_void_p(0)
+    _check(_load().cm_dg_diagnostics_static(C.byref(d), _dptr(Q_dev), _dptr(J_dev), _dptr(z_dev), sp, C.byref(out)),
+           "cm_dg_diagnostics_static")
+    return {k: getattr(out, k) for k, _ in _Diag._fields_}
 
 
 NPROF = 20   # CM_DG_NPROF

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1194,3 +1195,122 @@ int cm_dg_profile_end(cm_dg_ctx* ctx, cm_dg_kernel_stats* out) {
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------ a6 without a ctx: cm_dg_diagnostics_static
+// For callers that may not obtain device memory (a pool that owns the whole GPU, an attached monitor without a budget, a
+// loop that cannot afford cudaMalloc's device-wide synchronisation; see include/cm_dg.h): the partial sums that
+// cm_dg_diagnostics keeps in ctx-owned cudaMalloc'd buffers live here in one array built into the library image.
+// Layout in doubles: [0, 8) totals | [8, 8 + 7*256) block sums | then 7 per element, CM_DG_STATIC_MAX_ELEM elements.
+// Every device that loads this module carries the array until the process ends.
+static __device__ __align__(256) double cm_static_scratch[CM_DG_STATIC_SCRATCH_BYTES / sizeof(double)];
+
+namespace {
+
+struct DiagStaticArgs {
+  int Nq, Np, nvar;
+  long long stride;
+  const double* Q; const double* J; const double* z;
+  double w[CM_MAXNQ];
+  double R_d, c_vd, a, b, T_0, I_v0, grav;   // a = R_v - R_d, b = c_vv - c_vd (eq. 7-8)
+};
+
+// diag_kernel with the Jacobian determinant and the height read from caller arrays (no ctx geometry, no z table):
+// per-element sums {mass, energy, water, M |u|^2 / 2, M, max(|u| + c), non-finite count} into part[7 e ..].  `part` is the
+// DEVICE address of cm_static_scratch as returned by cudaGetSymbolAddress, handed in by the host like any other pointer.
+__global__ void diag_static_kernel(const __grid_constant__ DiagStaticArgs a, double* __restrict__ part) {
+  extern __shared__ double sh[];
+  const long long e = blockIdx.x;
+  double s[7] = {0, 0, 0, 0, 0, 0, 0};
+  for (int n = threadIdx.x; n < a.Np; n += blockDim.x) {
+    const int i = n % a.Nq, j = (n / a.Nq) % a.Nq, k = n / (a.Nq * a.Nq);
+    const long long idx = e * a.Np + n;
+    double Y[6] = {0, 0, 0, 0, 0, 0};
+    for (int v = 0; v < a.nvar; ++v) { Y[v] = a.Q[v * a.stride + idx]; if (!isfinite(Y[v])) s[6] += 1.0; }
+    const double M = a.w[i] * a.w[j] * a.w[k] * a.J[idx];
+    const double Phi = a.grav * a.z[idx];
+    const double ir = 1.0 / Y[0];
+    const double u2 = (Y[1] * Y[1] + Y[2] * Y[2] + Y[3] * Y[3]) * ir * ir;
+    const double q = (a.nvar == 6) ? Y[5] * ir : 0.0;
+    const double cvm = a.c_vd + a.b * q, Rm = a.R_d + a.a * q;
+    const double eint = Y[4] * ir - 0.5 * u2 - Phi;
+    const double T = a.T_0 + (eint - q * a.I_v0) / cvm;
+    const double c = sqrt((1.0 + Rm / cvm) * Rm * T);
+    s[0] += M * Y[0]; s[1] += M * Y[4]; s[2] += M * Y[5]; s[3] += M * 0.5 * u2; s[4] += M;
+    s[5] = fmax(s[5], sqrt(u2) + c);
+  }
+  for (int m = 0; m < 7; ++m) sh[m * blockDim.x + threadIdx.x] = s[m];
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double r[7] = {0, 0, 0, 0, 0, 0, 0};
+    for (int t = 0; t < blockDim.x; ++t)
+      for (int m = 0; m < 7; ++m) r[m] = (m == 5) ? fmax(r[m], sh[m * blockDim.x + t]) : r[m] + sh[m * blockDim.x + t];
+    for (int m = 0; m < 7; ++m) part[7 * e + m] = r[m];
+  }
+}
+
+// Device address of cm_static_scratch on the current device.  In host code the name `cm_static_scratch` is only a handle for
+// the runtime's symbol table (passing it to a kernel would hand the GPU a host address), so the address is asked for once
+// per device with that device current, checked, and remembered.  Devices beyond the table are looked up on every call.
+constexpr int kStaticMaxDev = 64;
+std::mutex g_static_mu;
+double* g_static_ptr[kStaticMaxDev] = {nullptr};
+
+int static_scratch(double** out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0)
+    return fail(CM_DG_ECUDA, "cm_dg_diagnostics_static: no current CUDA device (this library has no CPU path)");
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (dev < kStaticMaxDev && g_static_ptr[dev]) { *out = g_static_ptr[dev]; return CM_DG_OK; }
+  double* ptr = nullptr;
+  const cudaError_t err = cudaGetSymbolAddress((void**)&ptr, cm_static_scratch);
+  if (err != cudaSuccess || !ptr)
+    return fail(CM_DG_ECUDA, std::string("cm_dg_diagnostics_static: cudaGetSymbolAddress(cm_static_scratch) on device ") +
+                             std::to_string(dev) + ": " + cudaGetErrorString(err));
+  if (dev < kStaticMaxDev) g_static_ptr[dev] = ptr;
+  *out = ptr;
+  return CM_DG_OK;
+}
+
+}  // namespace
+
+extern "C" int cm_dg_diagnostics_static(const cm_dg_static_desc* d, const double* Q_dev, const double* J_dev, const double* z_dev,
+                                        void* cuda_stream, cm_dg_diag* out) {
+  if (!d || !Q_dev || !J_dev || !z_dev || !out) return fail(CM_DG_EINVAL, "cm_dg_diagnostics_static: NULL argument");
+  if (d->N < 1 || d->N > 7) return fail(CM_DG_EINVAL, "cm_dg_diagnostics_static: polynomial order N must be in 1..7");
+  if (d->nvar != 5 && d->nvar != 6) return fail(CM_DG_EINVAL, "cm_dg_diagnostics_static: nvar must be 5 or 6");
+  if (d->n_elem < 1) return fail(CM_DG_EINVAL, "cm_dg_diagnostics_static: n_elem must be >= 1");
+  if (d->n_elem > CM_DG_STATIC_MAX_ELEM)
+    return fail(CM_DG_EINVAL, "cm_dg_diagnostics_static: n_elem = " + std::to_string((long long)d->n_elem) +
+                              " exceeds CM_DG_STATIC_MAX_ELEM = " + std::to_string(CM_DG_STATIC_MAX_ELEM) +
+                              " (the built-in scratch array holds 7 sums per element and cannot grow; use cm_dg_diagnostics"
+                              " on a ctx for larger meshes)");
+  const int Nq = d->N + 1, Np = Nq * Nq * Nq;
+  if (d->field_stride < d->n_elem * Np) return fail(CM_DG_EINVAL, "cm_dg_diagnostics_static: field_stride is smaller than n_elem * (N+1)^3");
+  if (!(d->c_vd > 0.0) || !(d->R_d > 0.0)) return fail(CM_DG_EINVAL, "cm_dg_diagnostics_static: R_d and c_vd must be positive");
+  double* scratch = nullptr;
+  { int rc_ = static_scratch(&scratch); if (rc_) return rc_; }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  DiagStaticArgs a;
+  a.Nq = Nq; a.Np = Np; a.nvar = d->nvar; a.stride = d->field_stride; a.Q = Q_dev; a.J = J_dev; a.z = z_dev;
+  {
+    double xi[CM_MAXNQ], D[CM_MAXNQ][CM_MAXNQ];
+    for (int i = 0; i < CM_MAXNQ; ++i) a.w[i] = 0.0;
+    lgl_operators(d->N, xi, a.w, D);
+  }
+  a.R_d = d->R_d; a.c_vd = d->c_vd; a.a = d->R_v - d->R_d; a.b = d->c_vv - d->c_vd; a.T_0 = d->T_0; a.I_v0 = d->I_v0; a.grav = d->grav;
+  double* total = scratch; double* blk = scratch + 8; double* part = scratch + 8 + 7 * 256;
+  const int thr = 128, nb = 256;
+  diag_static_kernel<<<(unsigned)d->n_elem, thr, 7 * thr * sizeof(double), st>>>(a, part);
+  CM_CUDA(cudaGetLastError());
+  // the same two fixed-order stages as cm_dg_diagnostics; all nb block rows and all 7 totals are rewritten on every call
+  const long long chunk = (d->n_elem + nb - 1) / nb;
+  diag_reduce_kernel<<<nb, 256, 0, st>>>(d->n_elem, chunk, part, blk);
+  diag_reduce_kernel<<<1, 256, 0, st>>>(nb, nb, blk, total);
+  CM_CUDA(cudaGetLastError());
+  double s[7] = {0, 0, 0, 0, 0, 0, 0};
+  CM_CUDA(cudaMemcpyAsync(s, total, sizeof(s), cudaMemcpyDeviceToHost, st));
+  CM_CUDA(cudaStreamSynchronize(st));
+  out->mass = s[0]; out->energy = s[1]; out->water = s[2]; out->kinetic = s[3] / s[4]; out->volume = s[4];
+  out->max_wavespeed = s[5]; out->n_nonfinite = (int64_t)s[6]; out->min_node_dx = 0.0;
+  return CM_DG_OK;
+}

@@ -56,6 +56,20 @@ def test_argument_validation_precedes_device_use():
         P.cm_dg_setup(bad)
 
 
+def test_static_diagnostics_checks_its_limit_before_device_use():
+    """cm_dg_diagnostics_static (built-in scratch array, for callers that cannot cudaMalloc) refuses a mesh beyond
+    CM_DG_STATIC_MAX_ELEM with a message naming the limit, before anything touches a device."""
+    import paper_2110_00853_b200 as P
+    import workloads as W
+    cfg, Q, dt = W.config1()
+    text = open(os.path.join(ROOT, "include", "cm_dg.h")).read()
+    assert int(re.search(r"#define CM_DG_STATIC_MAX_ELEM (\d+)", text).group(1)) == P.binding.STATIC_MAX_ELEM
+    with pytest.raises(P.CmDgError, match="exceeds CM_DG_STATIC_MAX_ELEM = %d" % P.binding.STATIC_MAX_ELEM):
+        P.cm_dg_diagnostics_static(cfg, P.binding.STATIC_MAX_ELEM + 1, 2 ** 40, 256, 256, 256)
+    with pytest.raises(P.CmDgError, match="NULL"):
+        P.cm_dg_diagnostics_static(cfg, 8, 8 * 125, 0, 256, 256)
+
+
 def test_product_does_not_import_oracle():
     pkg = os.path.join(ROOT, "paper_2110_00853_b200")
     for dp, _, files in os.walk(pkg):
