@@ -81,7 +81,7 @@ typedef struct {
                                with u_p,int the wall-parallel velocity at the first layer of interior nodes          */
   double lhf_bottom;        /* W m^-2 latent heat flux, added to shf_bottom in the wall energy flux   */
   double evap_bottom;       /* kg m^-2 s^-1 evaporation E = n.(rho d_qv)|sfc into the domain: enters the
-                               rho*q_tot and rho equations (nvar == 6); the caller derives it from LHF                */
+                               rho*q_tot and rho equations; CM_DG_EINVAL unless nvar == 6; the caller derives it from LHF */
   /* ---- equilibrium moist thermodynamics (section 2.7, eq. 15); nvar == 6; runs on the stored-metric kernels ---- */
   int32_t satadj;           /* 1: temperature and liquid water from the saturation adjustment: the root T of
                                I*(T; rho, q_tot) = I by Newton iterations, the saturation excess q_tot - q_v*(T, rho) as liquid
@@ -136,7 +136,7 @@ typedef struct {
 int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out);
 
 /* Same with explicit scheduling knobs (tuning == NULL: defaults).  CM_DG_EINVAL for an unknown kernel id or a row_len
- * that does not divide the x-chunk. */
+ * that does not divide the x-chunk.  After any refusal *out is NULL. */
 int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tuning, void* cuda_stream, cm_dg_ctx** out);
 
 /* Layout of state arrays: n_elem, np, field_stride (doubles) and, if non-NULL, lex_of_elem (HOST, n_elem

@@ -628,13 +628,13 @@ int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out) {
 
 int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cuda_stream, cm_dg_ctx** out) {
   if (!p || !out) return fail(CM_DG_EINVAL, "cm_dg_setup: NULL argument");
+  *out = nullptr;   // before the first early return: a refused setup never leaves a stale handle behind
   cm_dg_tuning tn;
   std::memset(&tn, 0, sizeof(tn));
   tn.ahead_t = tn.ahead_g = -1;
   if (tune) tn = *tune;
   if (tn.kernel != 0 && tn.kernel != 2 && tn.kernel != 7 && tn.kernel != 10 && tn.kernel != 11) return fail(CM_DG_EINVAL, "cm_dg_setup_tuned: kernel must be 0, 2, 7, 10 or 11");
   if (tn.max_chunk < 0 || tn.max_patch < 0 || tn.row_len < 0) return fail(CM_DG_EINVAL, "cm_dg_setup_tuned: negative tile size");
-  *out = nullptr;
   if (p->N < 2 || p->N > 7) return fail(CM_DG_EINVAL, "cm_dg_setup: polynomial order N must be in 2..7");
   if (p->nvar != 5 && p->nvar != 6) return fail(CM_DG_EINVAL, "cm_dg_setup: nvar must be 5 or 6");
   for (int d = 0; d < 3; ++d) {
@@ -664,6 +664,8 @@ int cm_dg_setup_tuned(const cm_dg_params* p, const cm_dg_tuning* tune, void* cud
   if (p->drag_cd < 0.0) return fail(CM_DG_EINVAL, "cm_dg_setup: drag_cd must be >= 0");
   if ((p->drag_cd != 0.0 || p->lhf_bottom != 0.0 || p->evap_bottom != 0.0) && p->bc[2] != 1)
     return fail(CM_DG_EINVAL, "cm_dg_setup: surface fluxes (drag_cd, lhf_bottom, evap_bottom) need a wall in z (bc[2] == 1)");
+  if (p->evap_bottom != 0.0 && p->nvar != 6)
+    return fail(CM_DG_EINVAL, "cm_dg_setup: evap_bottom needs the moisture tracer (nvar == 6): a dry run would drop the prescribed mass and water flux");
   const int64_t Ne = (int64_t)p->ne[0] * p->ne[1] * p->ne[2];
   const int Nq = p->N + 1, Np = Nq * Nq * Nq;
   if (Ne * Np >= (int64_t)1 << 31) return fail(CM_DG_EINVAL, "cm_dg_setup: more than 2^31 nodes");

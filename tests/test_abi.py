@@ -54,6 +54,22 @@ def test_argument_validation_precedes_device_use():
     bad = dict(cfg); bad["bc"] = (0, 2, 0)
     with pytest.raises(P.CmDgError, match="bc"):
         P.cm_dg_setup(bad)
+    # prescribed evaporation enters rho and rho*q_tot: a dry state (nvar == 5) cannot carry it
+    bad = dict(cfg); bad["bc"] = (0, 0, 1); bad["nvar"] = 5; bad["evap_bottom"] = 1e-5
+    with pytest.raises(P.CmDgError, match="evap_bottom needs the moisture tracer"):
+        P.cm_dg_setup(bad)
+
+
+def test_refused_setup_clears_the_handle():
+    """*out is NULL after every refusal, also one caused by the tuning struct (checked first)."""
+    import ctypes as C
+    from paper_2110_00853_b200 import binding as B
+    L = B._load()
+    p = B._Params(); p.N = 4
+    tn = B._Tuning(kernel=5, ahead_t=-1, ahead_g=-1)
+    ctx = C.c_void_p(0xdead)
+    assert L.cm_dg_setup_tuned(C.byref(p), C.byref(tn), None, C.byref(ctx)) == -1
+    assert not ctx.value
 
 
 def test_static_diagnostics_checks_its_limit_before_device_use():
