@@ -521,9 +521,11 @@ struct cm_dg_ctx {
   int tileL = 1, tilePY = 1;       // the tiled element order (x-chunk, y-patch)
   // one time step as a CUDA graph: captured on the second consecutive call with the same state array, dt and coefficient
   // table, replayed afterwards (the 10-12 launches of a step are launch-bound on small meshes)
+  // the key holds the coefficient table itself: A_s, B_s and dt are baked into the captured kernel arguments, so two tables
+  // may share a graph only if every entry is equal (a checksum could collide and replay stale coefficients silently)
   struct StepKey {
-    const double* Q = nullptr; double dt = 0.0; int nstages = 0; double tab = 0.0;
-    bool operator==(const StepKey& o) const { return Q == o.Q && dt == o.dt && nstages == o.nstages && tab == o.tab; }
+    const double* Q = nullptr; double dt = 0.0; int nstages = 0; std::vector<double> A, B;
+    bool operator==(const StepKey& o) const { return Q == o.Q && dt == o.dt && nstages == o.nstages && A == o.A && B == o.B; }
   };
   bool graphs = true;
   cudaGraphExec_t step_exec = nullptr;
@@ -1044,7 +1046,7 @@ int cm_dg_lsrk_step_table(cm_dg_ctx* ctx, double* Q_dev, double t, double dt, in
   if (ctx->graphs && !ctx->profiling && nsteps > 0) {
     cm_dg_ctx::StepKey key;
     key.Q = Q_dev; key.dt = dt; key.nstages = nstages;
-    for (int s = 0; s < nstages; ++s) key.tab += (s + 1) * (A[s] + 3.0 * B[s]);
+    key.A.assign(A, A + nstages); key.B.assign(B, B + nstages);
     if (ctx->step_exec && key == ctx->step_key) {
       for (int s = 0; s < nsteps; ++s) CM_CUDA(cudaGraphLaunch(ctx->step_exec, ctx->st));
       return CM_DG_OK;
