@@ -321,6 +321,11 @@ __global__ void __launch_bounds__(CmCfg7<Nq, MOIST>::THREADS + 32, CmCfg10<Nq, M
     // releases the buffers of the previous iteration to the producer WITHOUT waiting: a warp that has finished phase 3
     // starts phase 1 of the next element at once.  What phase 1 writes is either private to the thread's own node (F^2,
     // c) or lies in the other tile buffer; the xi- carry is written behind the first compute barrier for this reason.
+    // Every compute thread orders its own generic-proxy stores to the buffers (F^1 / F^3 over G, the xi carry, the face
+    // results) before the async-proxy bulk copies that will overwrite them: the PTX memory model makes a proxy fence
+    // cover only the executing thread's prior accesses, so the fence must run in the writers before they signal the
+    // producer (the pattern of a TMA-store fence), not only in the producer after the barrier.
+    cm10_fence_proxy_async();
     cm10_bar_release(THREADS + 32);
     cm7_mbar_wait(mbar + b, (it >> 1) & 1);
 
