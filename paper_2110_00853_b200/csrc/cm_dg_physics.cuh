@@ -69,18 +69,34 @@ __device__ __forceinline__ double cm_sat_q(const CmThermo& th, double T, double 
   const double iT = 1.0 / T;
   return th.p_tr * pow(T * th.iT_tr, th.sx1) * exp(th.sx2 * (th.iT_tr - iT)) * iT / (rho * th.R_v);
 }
+// Safeguard: the root is bracketed from the start and the bracket shrinks with the sign of f at every iterate.
+//   lo = unsaturated T: there the excess is still vapour, condensing it releases (c_vv - c_vl)(T - T_0) + I_v0 > 0 per
+//        unit of water, so I*(lo) < I and f(lo) < 0;
+//   hi = T with all of q_t liquid, T_0 + I / ((1 - q_t) c_vd + q_t c_vl): I*(T) - I_liquid(T) = q_v [(c_vv - c_vl)(T - T_0)
+//        + I_v0] >= 0 for every T, so f(hi) >= 0.
+// A Newton step that leaves [lo, hi] (or is not a number) is replaced by the midpoint, so a finite state always converges
+// (bisection alone needs < 50 halvings of a bracket of tens of kelvin to reach 1e-14 T).  Iterates that stay inside, which
+// is every step on the tested states, are the plain Newton iterates.  If the loop ends unconverged all the same (non-finite
+// input), NaN is returned: it reaches the state and cm_dg_diagnostics counts it in n_nonfinite instead of a silently wrong
+// pressure.
 static __device__ __noinline__ double cm_sat_adjust(const CmThermo& th, double I, double rho, double qt, double& ql) {
   double T = th.T_0 + (I - qt * th.I_v0) / (th.c_vd + th.b * qt);
   if (qt <= cm_sat_q(th, T, rho)) { ql = 0.0; return T; }
-  for (int it = 0; it < 50; ++it) {
+  double lo = T, hi = th.T_0 + I / ((1.0 - qt) * th.c_vd + qt * th.c_vl);
+  bool conv = false;
+  for (int it = 0; it < 60; ++it) {
     const double qs = cm_sat_q(th, T, rho), dT0 = T - th.T_0;
     const double f = (1.0 - qt) * th.c_vd * dT0 + qs * (th.c_vv * dT0 + th.I_v0) + (qt - qs) * th.c_vl * dT0 - I;
     const double dqs = qs * ((th.Lv0 + th.dcp * dT0) / (th.R_v * T * T) - 1.0 / T);
     const double df = (1.0 - qt) * th.c_vd + qs * th.c_vv + (qt - qs) * th.c_vl + dqs * ((th.c_vv - th.c_vl) * dT0 + th.I_v0);
-    const double dT = f / df;
-    T -= dT;
-    if (fabs(dT) <= 1e-14 * T) break;
+    if (f < 0.0) lo = fmax(lo, T); else hi = fmin(hi, T);
+    double Tn = T - f / df;
+    if (!(Tn >= lo && Tn <= hi)) Tn = 0.5 * (lo + hi);
+    const double dT = T - Tn;
+    T = Tn;
+    if (fabs(dT) <= 1e-14 * T) { conv = true; break; }
   }
+  if (!conv) T = __longlong_as_double(0x7ff8000000000000LL);
   ql = qt - cm_sat_q(th, T, rho);
   return T;
 }

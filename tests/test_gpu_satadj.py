@@ -82,3 +82,29 @@ def test_satadj_needs_moisture(P):
     cfg, Q, dt = small_config(3)
     with pytest.raises(P.CmDgError):
         P.CmDg(dict(cfg, satadj=1))
+
+
+def test_satadj_extreme_states_converge(P, oracle_mod):
+    """The kernel's Newton iteration is bracketed (unsaturated T below, all-liquid T above, midpoint when a step leaves the
+    bracket) while the oracle runs the paper's plain Newton.  On states far outside the atmospheric range of the other
+    tests (215-325 K, 0.25-1.35 kg/m^3, q_t up to 0.08: three quarters of the nodes heavily supersaturated) both must land
+    on the same root: no non-finite value, and the pressure-dependent level statistics and the wave speed agree."""
+    cfg, Q, dt = small_config(5)
+    cfg = dict(cfg, satadj=1)
+    xyz = W.node_coords(cfg)
+    rng = np.random.default_rng(20211000)
+    shp = xyz[..., 2].shape
+    T = rng.uniform(215.0, 325.0, shp); rho = rng.uniform(0.25, 1.35, shp); q = rng.uniform(0.0, 0.08, shp)
+    u, v, w = (rng.uniform(-5.0, 5.0, shp) for _ in range(3))
+    Qx = W.conserved(cfg, rho, u, v, w, T, q, xyz[..., 2])
+    o = oracle_mod.Oracle(cfg); g = P.CmDg(cfg)
+    ql = np.array([o.primitives(Qx[e, 3], z=xyz[e, 3, 2], ref=None)["ql"] for e in range(o.Ne)])
+    assert (ql > 1e-3).mean() > 0.5 and (ql == 0).any()
+    Qd = g.to_device(Qx)
+    dg, do = g.diagnostics(Qd), o.diagnostics(Qx)
+    assert dg["n_nonfinite"] == 0
+    assert abs(dg["max_wavespeed"] - do["max_wavespeed"]) <= 1e-12 * do["max_wavespeed"]
+    Pg, Po = g.profiles(Qd), o.profiles(Qx)
+    for col in (5, 7):                                   # h_tot and theta_v carry the adjusted pressure of every node
+        assert np.max(np.abs(Pg[:, col] - Po[:, col])) <= 1e-12 * np.max(np.abs(Po[:, col])), col
+    g.close()
