@@ -97,6 +97,38 @@ def test_lsrk_table_parity(P, oracle_mod, k):
         g.lsrk_step_table(Qa, dt, 1, [0.5], [1.0])
 
 
+@pytest.mark.parametrize("k", [2, 5])
+def test_lsrk_table_14_stages(P, oracle_mod, k):
+    """The paper's runs use a 14-stage 2N-storage scheme (its coefficients are not in this repository).  The table
+    entry point at nstages = 14: (a) 14 forward-Euler sub-steps (A = 0, B = 1/14) and (b) the (5,4) table behind nine
+    zero-weight stages, both against the oracle's plain recurrence; (b) must also reproduce cm_dg_lsrk_step bit for bit
+    (a stage with B_s = 0 leaves U as it is and the first real stage has A = 0).  Then the same 14-stage step replayed from
+    its CUDA graph (28 kernel launches on the closure configs) against plain launches."""
+    import torch
+    cfg, Q, dt = small_config(k)
+    o = oracle_mod.Oracle(cfg); g = P.CmDg(cfg)
+    A5, B5, _ = oracle_mod.lsrk54_coeffs()
+    euler = (np.zeros(14), np.full(14, 1.0 / 14.0))
+    padded = (np.concatenate([np.zeros(9), A5]), np.concatenate([np.zeros(9), B5]))
+    for name, (A, B), n in (("euler", euler, 6), ("padded", padded, 6)):
+        Qd = g.to_device(Q); g.lsrk_step_table(Qd, 0.5 * dt, n, A, B)
+        err = state_errors(g.to_host(Qd), o.lsrk_table(Q, 0.5 * dt, n, A, B))
+        assert np.all(err <= STEP_TOL), (name, err)
+    Qa = g.to_device(Q); g.lsrk_step_table(Qa, dt, 3, *padded)
+    Qb = g.to_device(Q); g.lsrk_step(Qb, dt, 3)
+    assert bool((Qa == Qb).all())
+    g.close()
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        ga = P.CmDg(cfg, stream=stream); gb = P.CmDg(cfg, stream=stream, tuning={"no_graph": 1})
+        Qa, Qb = ga.to_device(Q), gb.to_device(Q)
+        for _ in range(4):                                # direct, capture, replay, replay
+            ga.lsrk_step_table(Qa, 0.5 * dt, 2, *euler); gb.lsrk_step_table(Qb, 0.5 * dt, 2, *euler)
+        stream.synchronize()
+        assert torch.equal(Qa, Qb)
+    ga.close(); gb.close()
+
+
 @pytest.mark.parametrize("k", [1, 3, 4, 5])
 def test_hllc_parity(P, oracle_mod, k):
     cfg, Q, dt = small_config(k)
