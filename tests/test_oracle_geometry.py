@@ -52,6 +52,43 @@ def test_flat_metrics(oracle_mod):
     assert abs(o.mass().sum() - 3.0 * 2.0 * 6.0) < 1e-12
 
 
+def test_flat_metrics_far_from_the_origin(oracle_mod):
+    """Eq. (24), on a flat brick that sits where config 4's last elements sit: 2.9e5 m from the origin in x
+    (and 1.2e5 m in y), 2500 m x 700 m elements, N = 4.  D annihilates constants, so differentiating the coordinates
+    relative to the element's first node is eq. (24) unchanged; in floating point it is not: products D_im x_m that carry
+    the offset leave sum_m D_im x_m = x * (rounding of the row sum of D) ~ 3e5 * 1e-16 where the exact derivative is 0, i.e.
+    spurious off-diagonal metric terms of relative size ~ eps |x| / h and a free-stream residual of the same size.
+    Pinned here (measured with the element-relative form / with absolute coordinates, i.e. with the `- x[d]` terms of
+    elem_geo_compute removed; the second column fails):
+      off-diagonal Ja entries  <= 32 eps max|Ja_dd|        6.6 eps  / 1270 eps
+      uniform-flow tendency    <  1e-13 T_f per field      4.8e-15  / 8.4e-13
+    The diagonal entries and J meet their closed forms to 16 eps |x| / h (the nodal coordinates themselves are rounded at
+    ulp(3e5) = 6e-11 on a 700 m element, which no differentiation can undo)."""
+    hx, hy, hz = 2500.0, 2500.0, 700.0
+    lo = (2.9e5, 1.2e5, 0.0)
+    cfg = W.base_params(N=4, ne=(4, 2, 3), lo=lo, hi=(lo[0] + 4 * hx, lo[1] + 2 * hy, 3 * hz), bc=(0, 0, 0), grav=0.0)
+    o = oracle_mod.Oracle(cfg)
+    eps = np.finfo(float).eps
+    want = np.array([hy * hz / 4, hx * hz / 4, hx * hy / 4])
+    off = ~np.eye(3, dtype=bool)
+    rel = 16 * eps * (lo[0] + 4 * hx) / hz
+    for e in range(o.Ne):
+        g = o.elem_geometry(e)
+        assert np.max(np.abs(g["Ja"][:, off])) <= 32 * eps * want.max(), e
+        for d in range(3):
+            assert np.max(np.abs(g["Ja"][:, d, d] - want[d])) <= rel * want[d], (e, d)
+        assert np.max(np.abs(g["J"] - hx * hy * hz / 8)) <= rel * hx * hy * hz / 8, e
+    z = o.coords()[..., 2]
+    one = np.ones_like(z)
+    Q = W.conserved(cfg, 1.1 * one, 12.0 * one, -7.0 * one, 3.0 * one, 288.0 * one, 0.0 * one, z)
+    dx = o.diagnostics(Q)["min_node_dx"]
+    for form in ("weak", "strong"):
+        dQ = o.rhs(Q, form)
+        for v in range(cfg["nvar"]):
+            Tf = max(abs(np.array(o.flux1(Q[0, 0])[v]).max()), 1e-300) / dx
+            assert np.max(np.abs(dQ[..., v])) < 1e-13 * Tf, (form, v)
+
+
 @pytest.mark.parametrize("maker", [_warped_cfg, _general_cfg])
 def test_warped_metrics(oracle_mod, maker):
     cfg = maker()
