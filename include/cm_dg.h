@@ -47,7 +47,11 @@ typedef struct cm_dg_ctx cm_dg_ctx; /* opaque, library-owned */
 
 /* Problem description (all HOST memory, copied before cm_dg_setup returns). */
 typedef struct {
-  int32_t N;                /* polynomial order, 2..7 (the paper and BASELINE use 4; sweep 3..6)            */
+  int32_t N;                /* polynomial order, 2..7 (the paper's runs and BASELINE use 4; the
+                               sweep 3..6).  N = 1 is refused with CM_DG_EINVAL: with two LGL nodes per direction every node
+                               lies on three faces, the drag law's "first layer of interior nodes" (A2) does not exist, and
+                               the kernels' split into volume lines and face nodes has no interior left to overlap with;
+                               no configuration of the paper or of BASELINE uses it                              */
   int32_t ne[3];            /* Ex, Ey, Ez: structured hexahedral brick                             */
   double lo[3], hi[3];      /* domain box before warping [m]                                                */
   int32_t bc[3];            /* per direction: 0 periodic, 1 impenetrable free-slip no-flux wall at both ends */
@@ -132,7 +136,8 @@ typedef struct {
 
 /* a0: mesh, LGL nodes/weights, derivative matrix, metric terms (eq. 24), connectivity,
  * reference state.  `cuda_stream` is a cudaStream_t (NULL = default stream).  On success *out owns all
- * device scratch (geometry, gradient array, LSRK residual, two more state buffers). */
+ * device scratch (geometry, gradient array, LSRK residual, two more state buffers); the one exception is the staging
+ * buffer of the *_host calls, see there. */
 int cm_dg_setup(const cm_dg_params* p, void* cuda_stream, cm_dg_ctx** out);
 
 /* Same with explicit scheduling knobs (tuning == NULL: defaults).  CM_DG_EINVAL for an unknown kernel id or a row_len
@@ -233,7 +238,10 @@ int cm_dg_diagnostics_static(const cm_dg_static_desc* desc, const double* Q_dev,
 int cm_dg_profiles(cm_dg_ctx* ctx, const double* Q_dev, double* out_host, int32_t nlev_capacity);
 
 /* End-to-end variants on HOST buffers in the same [nvar][field_stride] layout (pinned memory recommended):
- * host->device copy, the device call above, device->host copy, stream synchronise. */
+ * host->device copy, the device call above, device->host copy, stream synchronise.  The device staging buffer
+ * (2 x nvar x field_stride doubles) is NOT part of what cm_dg_setup allocates: the first *_host call on a ctx cudaMallocs it
+ * (CM_DG_ENOMEM if that fails) and cm_dg_destroy frees it, so a ctx that is only ever driven with device pointers does not
+ * pay for it.  Make that first call outside any stream capture and outside a timed region. */
 int cm_dg_rhs_host(cm_dg_ctx* ctx, const double* Q_host, double* dQ_host, double t);
 int cm_dg_lsrk_step_host(cm_dg_ctx* ctx, double* Q_host, double t, double dt, int32_t nsteps);
 
