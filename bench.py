@@ -296,6 +296,32 @@ LEGS = {
 }
 
 
+def _next_leg(**over):
+    """Config 5 on a 48x48x48 cut (13.8 M nodes, state 0.66 GB per copy: still far larger than L2) with one of the further
+    options switched on: the throughput of the scope table's NEXT rows."""
+    def make(W):
+        if not _C5CUT_CACHE:
+            _C5CUT_CACHE.append(W.config5(ne=(48, 48, 48), N=4, hi=(3000.0, 3000.0, 3000.0)))   # the same seeded state for every leg
+        cfg, Q, dt = _C5CUT_CACHE[0]
+        return dict(cfg, **over), Q, dt
+    return make
+
+
+_C5CUT_CACHE = []
+
+
+_C5CUT = "config 5 cut 48x48x48, N=4, "
+LEGS.update({
+    "c5_vreman": (_next_leg(sgs=2, richardson=1), 3, _C5CUT + "Vreman closure + Richardson factor (NEXT-1)", (6, 1, False)),
+    "c5_sponge_filter": (_next_leg(sponge_alpha=0.4, sponge_zs=2400.0, filter_order=64), 3, _C5CUT + "Rayleigh sponge + exponential filter after every step (NEXT-2)", (6, 1, False)),
+    "c5_hllc": (_next_leg(riemann=1), 3, _C5CUT + "HLLC flux (NEXT-3; thread-per-node kernels)", (6, 1, False)),
+    "c5_roe": (_next_leg(riemann=2), 3, _C5CUT + "Roe flux (NEXT-3; thread-per-node kernels)", (6, 1, False)),
+    "c5_satadj": (_next_leg(satadj=1), 3, _C5CUT + "saturation-adjusted equation of state (NEXT-4; thread-per-node kernels)", (6, 1, False)),
+    "c5_surface": (_next_leg(drag_cd=1.3e-3, lhf_bottom=147.2, evap_bottom=5.9e-5), 3, _C5CUT + "drag law + LHF + evaporation at the bottom wall (NEXT-4)", (6, 1, False)),
+})
+NEXT_LEGS = ("c5_vreman", "c5_sponge_filter", "c5_hllc", "c5_roe", "c5_satadj", "c5_surface")
+
+
 def one_leg(P, torch, name, peak, tuning=None):
     """One of the further workloads by name (also `bench.py --leg NAME`, the command the ncu captures of the stored-metric
     kernels run).  For the stored-metric legs the bytes those kernels really move are reported beside the algorithmic
@@ -332,6 +358,7 @@ def extra_legs(P, torch, args, peak):
         del cfg, Q
     for name in ("c2", "c3", "c3x", "c4", "c4x", "c4s"):
         out["configs"].append(one_leg(P, torch, name, peak))
+    out["next_rows"] = [one_leg(P, torch, name, peak) for name in NEXT_LEGS]
     return out
 
 
@@ -503,6 +530,8 @@ def run_ours(args):
         line["extra"] = extra_legs(P, torch, args, peak)
         for leg in line["extra"]["sweep"]:
             roof["sweep_N%d_frac" % leg["order"]] = leg["frac_of_measured_hbm"]
+        for leg in line["extra"]["next_rows"]:
+            roof["%s_gdofs" % leg["leg"]] = leg["value"] / 1e9
         for leg in line["extra"]["configs"]:
             if leg.get("leg") in ("c2", "c3", "c4"):     # launch-bound meshes: graph replay against plain launches
                 roof["%s_ms_per_step_graph" % leg["leg"]] = leg["ms_per_step"]
