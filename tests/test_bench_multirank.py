@@ -45,3 +45,23 @@ def test_single_rank_is_identity():
     import bench
     value, ms = bench.whole_job_value(1000, 2, 8.0, 1, None, None)
     assert ms == 8.0 and abs(value - 1000 * 5 * 2 / 8.0e-3) < 1e-9 * value
+
+
+def test_bench_legs_are_well_formed():
+    """Host logic of bench.py's further workloads: every NEXT-row leg exists, builds its config on the shared 48x48x48 cut of
+    config 5 with exactly the option it names switched on, and carries a positive algorithmic byte count."""
+    import bench
+    import workloads as W
+    assert set(bench.NEXT_LEGS) <= set(bench.LEGS)
+    want = {"c5_vreman": {"sgs": 2, "richardson": 1}, "c5_hllc": {"riemann": 1}, "c5_roe": {"riemann": 2},
+            "c5_satadj": {"satadj": 1}, "c5_sponge_filter": {"filter_order": 64}, "c5_surface": {"drag_cd": 1.3e-3}}
+    base = None
+    for name in bench.NEXT_LEGS:
+        make, steps, label, sb = bench.LEGS[name]
+        cfg, Q, dt = make(W)
+        assert tuple(cfg["ne"]) == (48, 48, 48) and cfg["N"] == 4 and cfg["nvar"] == 6 and steps >= 3
+        for k, v in want[name].items():
+            assert cfg[k] == v, (name, k)
+        assert bench.stage_bytes(*sb) > 0 and "48x48x48" in label
+        base = Q if base is None else base
+        assert Q is base                                  # one seeded state shared by the legs
